@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- advection grid-points/sec and achieved HBM GB/s on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload config1|config2|config3] [--xchunk X] [--group G]
+
+A "step" is one pass of the hot path over one batch of synthetic fields:
+  config1 (default, the configuration BASELINE.json's metric is quoted on):
+      256x256x128 fp64, one fused u/v/w momentum call;
+  config2 / config3: 512x512x256, momentum + 10 batched scalars (a1 + a2),
+      fp64 / fp32 (a4).
+`value` is interior grid points advected per second with inputs resident in
+HBM; `e2e` is the same metric through monc_adv_step_async with PINNED HOST
+buffers (H2D of the fields, kernels, D2H of the tendencies inside the timed
+region).  Prints ONE JSON line (rank 0).
+
+--impl reference times the CPU oracle (oracle/, fp64, single thread) on the
+same workload: each step is one full oracle pass over the first `--ref-planes`
+x planes of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+# algorithmic bytes per interior point: every input read
+# once, every output written once
+BYTES_PER_PT = {"momentum": {"f64": 48, "f32": 24}}
+
+
+def scalar_bytes_per_pt(nq, dtype):
+    es = 8 if dtype == "f64" else 4
+    return 3 * es + 2 * es * nq  # wind once + q in + sq out
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_cfg(name):
+    from paper_2009_12850_b200 import synth
+    return synth.CONFIGS[{"config1": 1, "config2": 2, "config3": 3}[name]]
+
+
+# ---------------------------------------------------------------------------
+# reference arm: the CPU oracle as it stands
+# ---------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import dataclasses
+    import oracle
+    from paper_2009_12850_b200 import synth
+    cfg = workload_cfg(args.workload)
+    sub = dataclasses.replace(cfg, nx=min(cfg.nx, args.ref_planes))
+    g = synth.grid(cfg.nz)
+    P = oracle.Problem(sub.nx, sub.ny, sub.nz, sub.halo, synth.DX, synth.DY,
+                       g["dz"], g["dzn"], g["rho"], g["rhon"])
+    names = ["u", "v", "w"] + synth.field_names(sub)
+    H = [synth.field(sub, n) for n in names]
+    outs = tuple(np.zeros(P.shape) for _ in range(3))
+    sq = np.zeros(P.shape)
+
+    def step():
+        P.momentum(H[0], H[1], H[2], nthreads=1, out=outs)
+        for q in H[3:]:
+            P.scalar(H[0], H[1], H[2], q, nthreads=1, out=sq)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = sub.points * args.steps / dt / 1e9
+    sample = (f"oracle (fp64, 1 thread) on the first {sub.nx} of {cfg.nx} x-planes of {args.workload}"
+              f" ({sub.points} pts/step, {len(names)} fields)")
+    print(json.dumps({
+        "impl": "reference", "metric": "advection grid-points/sec", "value": val, "unit": "Gpts/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz,
+                   "nq": cfg.nq, "halo": cfg.halo},
+        "cpu_baseline": {"value": val, "unit": "Gpts/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "Gpts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2009_12850_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = workload_cfg(args.workload)
+    g = synth.grid(cfg.nz)
+    L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY,
+                        g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=cfg.dtype)
+    L.set_tuning(xchunk=args.xchunk, group=args.group)
+    if args.variant:
+        L.set_variant(args.variant)
+    tdt = L.torch_dtype
+    # weak scaling: every rank advects its own subdomain of the config's size
+    # ("replicas only" until the halo-exchange row of SURVEY.md 8(f) is built);
+    # rank-keyed seed so ranks do not share data
+    rcfg = cfg if rank == 0 else __import__("dataclasses").replace(cfg, seed_cid=1000 + rank)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(rcfg, n) for n in names]
+    nf = len(names)
+    field_bytes = cfg.elems * (8 if cfg.dtype == "f64" else 4)
+    # rotate between buffer sets so that no step finds its inputs in L2
+    nsets = max(2, min(4, int(np.ceil(3 * 126e6 / (2 * nf * field_bytes))) + 1))
+    sets = []
+    for s in range(nsets):
+        ins = [torch.from_numpy(a).to("cuda", dtype=tdt) for a in H]
+        outs = [torch.zeros(L.shape, device="cuda", dtype=tdt) for _ in names]
+        sets.append((ins, outs))
+    st = torch.cuda.Stream()
+
+    def step(s):
+        ins, outs = sets[s % nsets]
+        L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
+        if nf > 3:
+            L.scalars(ins[3:], outs[3:], stream=st)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    with torch.cuda.stream(st):
+        for s in range(args.warmup):
+            step(s)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    n0 = L.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    with torch.cuda.stream(st):
+        ev[0].record(st)
+        for s in range(args.steps):
+            ins, outs = sets[(args.warmup + s) % nsets]
+            L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
+            ev[2 * s + 1].record(st)
+            if nf > 3:
+                L.scalars(ins[3:], outs[3:], stream=st)
+            ev[2 * s + 2].record(st)
+    barrier()
+    launches = L.launch_count() - n0
+    total_ms = ev[0].elapsed_time(ev[-1])
+    mom_ms = [ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps)]
+    sca_ms = [ev[2 * s + 1].elapsed_time(ev[2 * s + 2]) for s in range(args.steps)]
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * cfg.points * args.steps / (total_ms * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer entry point (a3)
+    hin = [torch.empty(L.shape, dtype=tdt, pin_memory=True) for _ in names]
+    for t_, a in zip(hin, H):
+        t_.copy_(torch.from_numpy(a))
+    hout = [torch.zeros(L.shape, dtype=tdt, pin_memory=True) for _ in names]
+    L.set_chunks(8)
+
+    def e2e_step():
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+        L.step_wait()
+
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    phase = L.step_times_ms()
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    es = 8 if cfg.dtype == "f64" else 4
+    plane_b = (cfg.ny + 2 * cfg.halo) * cfg.nz * es
+    h2d_b = nf * (cfg.nx + 2) * plane_b
+    d2h_b = nf * cfg.points * es
+    e2e_val = world * cfg.points * e2e_steps / e2e_s / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel
+    peak, peak_src = peaks()
+    mom_b = BYTES_PER_PT["momentum"][cfg.dtype] * cfg.points
+    sca_b = scalar_bytes_per_pt(cfg.nq, cfg.dtype) * cfg.points if cfg.nq else 0
+    mom_avg, sca_avg = float(np.mean(mom_ms)), float(np.mean(sca_ms))
+    if sca_b and sca_avg > mom_avg:
+        kern, kb, kms = "march_scalars", sca_b, sca_avg
+    else:
+        kern, kb, kms = "march_momentum", mom_b, mom_avg
+    achieved = kb / (kms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
+                "best_launch_ms": float(np.min(mom_ms if kern == "march_momentum" else sca_ms)),
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+    kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
+    if sca_b:
+        kernels.update({"scalars_ms": sca_avg, "scalars_GBs": sca_b / (sca_avg * 1e-3) / 1e9})
+
+    # ---- the oracle beside it: bounded sample on this box's host cores
+    cpu = cpu_baseline(cfg, args)
+
+    out = {
+        "metric": "advection grid-points/sec", "value": value, "unit": "Gpts/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
+        "data": "synthetic",
+        "config": {"workload": args.workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz,
+                   "halo": cfg.halo, "nq": cfg.nq, "fields_per_step": nf,
+                   "l2": f"rotating {nsets} buffer sets ({nsets * 2 * nf * field_bytes / 1e6:.0f} MB) > 126 MB L2",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "xchunk": args.xchunk, "group": args.group},
+        "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
+        "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
+                "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
+                "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
+                "phase_ms": phase, "chunks": 8},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(cfg, args):
+    import dataclasses
+    import oracle
+    from paper_2009_12850_b200 import synth
+    sub = dataclasses.replace(cfg, nx=min(cfg.nx, args.ref_planes))
+    g = synth.grid(cfg.nz)
+    P = oracle.Problem(sub.nx, sub.ny, sub.nz, sub.halo, synth.DX, synth.DY,
+                       g["dz"], g["dzn"], g["rho"], g["rhon"])
+    names = ["u", "v", "w"] + synth.field_names(sub)
+    H = [synth.field(sub, n) for n in names]
+    outs = tuple(np.zeros(P.shape) for _ in range(3))
+    sq = np.zeros(P.shape)
+    reps, t0 = 0, time.perf_counter()
+    while True:
+        P.momentum(H[0], H[1], H[2], nthreads=1, out=outs)
+        for q in H[3:]:
+            P.scalar(H[0], H[1], H[2], q, nthreads=1, out=sq)
+        reps += 1
+        dt = time.perf_counter() - t0
+        if dt > args.cpu_seconds:
+            break
+    return {"value": sub.points * reps / dt / 1e9, "unit": "Gpts/s", "cores": 1, "kind": "oracle",
+            "sample": f"{reps} oracle passes (fp64, 1 thread) over the first {sub.nx} of {cfg.nx}"
+                      f" x-planes of {args.workload}, {len(names)} fields, {dt:.1f} s",
+            "host_cores_available": len(os.sched_getaffinity(0))}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3"])
+    ap.add_argument("--xchunk", type=int, default=0)
+    ap.add_argument("--group", type=int, default=0)
+    ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march"])
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--ref-planes", type=int, default=64)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="ncu dram bytes per launch of the dominant kernel, if known")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,35 @@
+"""Build the C-ABI CUDA library in-tree for sm_100a.
+
+    python -m paper_2009_12850_b200.build [--force] [--verbose]
+
+Output: paper_2009_12850_b200/libmonc_adv.so (git-ignored; travels to the GPU
+box with the gpurun snapshot).  nvcc cross-compiles without a GPU.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libmonc_adv.so")
+SOURCES = [os.path.join(CSRC, "monc_adv.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, "monc_adv_kernels.cuh"),
+                  os.path.join(ROOT, "include", "monc_adv.h")]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+         "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if (not force and os.path.exists(LIB)
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)):
+        return LIB
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

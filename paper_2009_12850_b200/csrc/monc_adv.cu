@@ -1,0 +1,607 @@
+// monc_adv.cu -- C ABI (include/monc_adv.h) over the sm_100a kernels.
+//
+// Host side of the library: handle, one-time constant upload,
+// kernel launch configuration, and the hybrid asynchronous step (PAPER.md:75-83,
+// 99-101): chunked H2D -> kernels -> D2H on separate streams with events.
+// No torch types, no CPU compute fallback: if CUDA fails the call fails.
+#include "monc_adv.h"
+#include "monc_adv_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace monc;
+
+namespace {
+thread_local std::string g_create_error;
+}
+
+struct monc_adv_s {
+  int nx = 0, ny = 0, nz = 0, h = 0, dtype = 0;
+  int nxh = 0, nyh = 0;
+  double dx = 0, dy = 0;
+  size_t elems = 0, esize = 8;
+  int device = 0;
+  int sm_count = 148;
+  void *d_tz[4] = {nullptr, nullptr, nullptr, nullptr};  // tzc1, tzc2, tzd1, tzd2 (dtype)
+  std::vector<double> tz_host[4];                        // as stored on the device
+  const void *wind[3] = {nullptr, nullptr, nullptr};
+  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0;
+  int xchunk = 0, group = 0;
+  long launches = 0;
+  std::string err;
+  // ---- async step state
+  int nchunks = 8, overlap = 1;
+  int staged_nq = -1;
+  std::vector<void *> d_in, d_out;  // 3+nq each
+  cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
+  cudaEvent_t ev_user = nullptr, ev_in_begin = nullptr, ev_out_begin = nullptr;
+  std::vector<cudaEvent_t> ev_h2d, ev_kb, ev_ke, ev_d2h;
+  std::vector<int> chunk_a, chunk_b;  // interior-relative x ranges of the in-flight step
+  bool in_flight = false, have_times = false;
+  float times[4] = {0, 0, 0, 0};
+};
+
+namespace {
+
+int fail(monc_adv_t h, int code, const std::string &msg) {
+  if (h) h->err = msg;
+  return code;
+}
+int cuda_fail(monc_adv_t h, cudaError_t e, const char *what) {
+  return fail(h, e == cudaErrorMemoryAllocation ? MONC_ADV_ENOMEM : MONC_ADV_ECUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);    \
+  } while (0)
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <typename T>
+KParams<T> make_params(monc_adv_t h, int ia, int ib) {
+  KParams<T> p;
+  p.nx = h->nx; p.ny = h->ny; p.nz = h->nz; p.h = h->h;
+  p.nyh = h->nyh;
+  p.plane = (long long)h->nyh * h->nz;
+  p.ia = ia; p.ib = ib;
+  constexpr int NK = VecOf<T>::NK;
+  p.wzc = (h->nz / NK + 31) / 32;
+  p.units = h->ny * p.wzc;
+  p.xc = ib - ia;
+  p.accumulate = h->accumulate;
+  p.skew = h->form == MONC_ADV_FORM_PW_SKEW;
+  p.cx = (T)(1.0 / (4.0 * h->dx));
+  p.cy = (T)(1.0 / (4.0 * h->dy));
+  p.tzc1 = (const T *)h->d_tz[0]; p.tzc2 = (const T *)h->d_tz[1];
+  p.tzd1 = (const T *)h->d_tz[2]; p.tzd2 = (const T *)h->d_tz[3];
+  return p;
+}
+
+// march kernels need whole 16-byte vectors per column and the flux form
+template <typename T>
+bool use_march(monc_adv_t h) {
+  if (h->variant == 1) return false;
+  if (h->form != MONC_ADV_FORM_FLUX) return false;
+  return h->nz % VecOf<T>::NK == 0;
+}
+
+// planes per block: enough blocks to fill the chip about `waves` times
+int pick_xchunk(monc_adv_t h, int nplanes, int blocks_per_plane, int resident_per_sm,
+                int multiplicity) {
+  if (h->xchunk > 0) return std::min(h->xchunk, nplanes);
+  const long slots = (long)h->sm_count * resident_per_sm;
+  long want = std::max<long>(1, slots / std::max(1, blocks_per_plane * multiplicity));
+  int xc = (int)((nplanes + want - 1) / want);
+  xc = std::max(xc, std::min(nplanes, 16));
+  return std::min(xc, nplanes);
+}
+
+template <typename T>
+int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
+                    int ia, int ib, cudaStream_t st) {
+  if (ib <= ia) return MONC_ADV_OK;
+  KParams<T> p = make_params<T>(h, ia, ib);
+  if (use_march<T>(h)) {
+    const int bx = (p.units + kWarpsPerBlock - 1) / kWarpsPerBlock;
+    p.xc = pick_xchunk(h, ib - ia, bx, 2, 1);
+    dim3 grid(bx, (ib - ia + p.xc - 1) / p.xc);
+    march_momentum<T><<<grid, kWarpsPerBlock * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+  } else {
+    const long long n = (long long)(ib - ia) * h->ny * h->nz;
+    generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
+  }
+  CU(cudaGetLastError());
+  h->launches++;
+  return MONC_ADV_OK;
+}
+
+template <typename T, int G>
+void launch_march_scalars(const KParams<T> &p, const ScalarPtrs<T> &ptrs, int nq, dim3 grid,
+                          int ngroups, const T *u, const T *v, const T *w, cudaStream_t st) {
+  march_scalars<T, G><<<grid, kWarpsPerBlock * 32, 0, st>>>(p, ptrs, nq, ngroups, u, v, w);
+}
+
+template <typename T>
+int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void *const *q,
+                   void *const *sq, int nq, int ia, int ib, cudaStream_t st) {
+  if (ib <= ia || nq == 0) return MONC_ADV_OK;
+  KParams<T> p = make_params<T>(h, ia, ib);
+  ScalarPtrs<T> ptrs;
+  for (int n = 0; n < kMaxScalars; ++n) {
+    ptrs.q[n] = (const T *)q[n < nq ? n : 0];
+    ptrs.sq[n] = (T *)sq[n < nq ? n : 0];
+  }
+  if (use_march<T>(h)) {
+    int G = h->group > 0 ? std::min(h->group, 5) : (nq >= 5 ? 5 : nq);
+    G = std::min(G, nq);
+    const int ngroups = (nq + G - 1) / G;
+    const int bx = (p.units + kWarpsPerBlock - 1) / kWarpsPerBlock;
+    p.xc = pick_xchunk(h, ib - ia, bx, 2, ngroups);
+    dim3 grid(bx * ngroups, (ib - ia + p.xc - 1) / p.xc);
+    switch (G) {
+      case 1: launch_march_scalars<T, 1>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+      case 2: launch_march_scalars<T, 2>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+      case 3: launch_march_scalars<T, 3>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+      case 4: launch_march_scalars<T, 4>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+      default: launch_march_scalars<T, 5>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+    }
+  } else {
+    const long long n = (long long)(ib - ia) * h->ny * h->nz;
+    dim3 grid((unsigned)((n + 255) / 256), nq);
+    generic_scalars<T><<<grid, 256, 0, st>>>(p, ptrs, u, v, w);
+  }
+  CU(cudaGetLastError());
+  h->launches++;
+  return MONC_ADV_OK;
+}
+
+int check_handle(monc_adv_t h) {
+  if (!h) return MONC_ADV_EINVAL;
+  cudaError_t e = cudaSetDevice(h->device);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaSetDevice");
+  return MONC_ADV_OK;
+}
+
+void free_staging(monc_adv_t h) {
+  for (void *p : h->d_in) if (p) cudaFree(p);
+  for (void *p : h->d_out) if (p) cudaFree(p);
+  h->d_in.clear();
+  h->d_out.clear();
+  h->staged_nq = -1;
+}
+
+int ensure_async_objects(monc_adv_t h, int nq) {
+  if (!h->s_in) {
+    CU(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&h->s_k, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&h->ev_user, cudaEventDisableTiming));
+    CU(cudaEventCreate(&h->ev_in_begin));
+    CU(cudaEventCreate(&h->ev_out_begin));
+  }
+  while ((int)h->ev_h2d.size() < h->nchunks) {
+    cudaEvent_t a, b, c, d;
+    CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
+    CU(cudaEventCreate(&c)); CU(cudaEventCreate(&d));
+    h->ev_h2d.push_back(a); h->ev_kb.push_back(b);
+    h->ev_ke.push_back(c); h->ev_d2h.push_back(d);
+  }
+  if (h->staged_nq < nq) {
+    // grow: keep what exists, add the missing scalar buffers
+    const int have = h->staged_nq < 0 ? 0 : 3 + h->staged_nq;
+    const int want = 3 + nq;
+    h->d_in.resize(want, nullptr);
+    h->d_out.resize(want, nullptr);
+    const size_t bytes = h->elems * h->esize;
+    for (int n = have; n < want; ++n) {
+      cudaError_t e = cudaMalloc(&h->d_in[n], bytes);
+      if (e == cudaSuccess) e = cudaMalloc(&h->d_out[n], bytes);
+      if (e != cudaSuccess) {
+        cudaGetLastError();
+        free_staging(h);
+        return cuda_fail(h, e, "cudaMalloc(staging)");
+      }
+      // output halos are never written by kernels: define them once
+      CU(cudaMemset(h->d_out[n], 0, bytes));
+      // input planes beyond halo depth 1 are never copied: define them once
+      CU(cudaMemset(h->d_in[n], 0, bytes));
+    }
+    h->staged_nq = nq;
+  }
+  return MONC_ADV_OK;
+}
+
+template <typename T>
+int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw,
+                    const void *const *hq, int nq, void *hsu, void *hsv, void *hsw,
+                    void *const *hsq, cudaStream_t user) {
+  const bool mom = hsu != nullptr;
+  const int C = std::min(h->nchunks, h->nx);
+  const size_t es = sizeof(T);
+  const size_t plane_b = (size_t)h->nyh * h->nz * es;
+  const int nf = 3 + nq;
+  std::vector<const char *> hin(nf);
+  std::vector<char *> hout(nf);
+  hin[0] = (const char *)hu; hin[1] = (const char *)hv; hin[2] = (const char *)hw;
+  hout[0] = (char *)hsu; hout[1] = (char *)hsv; hout[2] = (char *)hsw;
+  for (int n = 0; n < nq; ++n) { hin[3 + n] = (const char *)hq[n]; hout[3 + n] = (char *)hsq[n]; }
+
+  cudaStream_t sin = h->s_in;
+  cudaStream_t sk = h->overlap ? h->s_k : h->s_in;
+  cudaStream_t sout = h->overlap ? h->s_out : h->s_in;
+
+  if (user) {
+    CU(cudaEventRecord(h->ev_user, user));
+    CU(cudaStreamWaitEvent(sin, h->ev_user, 0));
+  }
+  h->chunk_a.assign(C, 0);
+  h->chunk_b.assign(C, 0);
+  for (int c = 0; c < C; ++c) {
+    h->chunk_a[c] = (int)((long long)h->nx * c / C);
+    h->chunk_b[c] = (int)((long long)h->nx * (c + 1) / C);
+  }
+  const T *du = (const T *)h->d_in[0], *dv = (const T *)h->d_in[1], *dw = (const T *)h->d_in[2];
+  std::vector<const void *> dq(std::max(nq, 1));
+  std::vector<void *> dsq(std::max(nq, 1));
+  for (int n = 0; n < nq; ++n) { dq[n] = h->d_in[3 + n]; dsq[n] = h->d_out[3 + n]; }
+
+  CU(cudaEventRecord(h->ev_in_begin, sin));
+  // ---- H2D: planes [h-1, h+nx] split so that chunk c's kernels need chunks <= c only
+  auto h2d_chunk = [&](int c) -> int {
+    const int lo = (c == 0) ? h->h - 1 : h->h + h->chunk_b[c - 1] + 1;
+    const int hi = h->h + h->chunk_b[c] + 1;  // exclusive; includes the +1 plane
+    const size_t off = (size_t)lo * plane_b, bytes = (size_t)(hi - lo) * plane_b;
+    for (int n = 0; n < nf; ++n)
+      CU(cudaMemcpyAsync((char *)h->d_in[n] + off, hin[n] + off, bytes, cudaMemcpyHostToDevice, sin));
+    CU(cudaEventRecord(h->ev_h2d[c], sin));
+    return MONC_ADV_OK;
+  };
+  auto compute_chunk = [&](int c) -> int {
+    const int ia = h->h + h->chunk_a[c], ib = h->h + h->chunk_b[c];
+    if (h->overlap) CU(cudaStreamWaitEvent(sk, h->ev_h2d[c], 0));
+    CU(cudaEventRecord(h->ev_kb[c], sk));
+    int rc = MONC_ADV_OK;
+    if (mom)
+      rc = launch_momentum<T>(h, du, dv, dw, (T *)h->d_out[0], (T *)h->d_out[1],
+                              (T *)h->d_out[2], ia, ib, sk);
+    if (rc == MONC_ADV_OK && nq > 0)
+      rc = launch_scalars<T>(h, du, dv, dw, dq.data(), dsq.data(), nq, ia, ib, sk);
+    if (rc != MONC_ADV_OK) return rc;
+    CU(cudaEventRecord(h->ev_ke[c], sk));
+    return MONC_ADV_OK;
+  };
+  auto d2h_chunk = [&](int c) -> int {
+    const int ia = h->h + h->chunk_a[c], ib = h->h + h->chunk_b[c];
+    if (h->overlap) CU(cudaStreamWaitEvent(sout, h->ev_ke[c], 0));
+    if (c == 0) CU(cudaEventRecord(h->ev_out_begin, sout));
+    // interior columns only: 2-D copy, one row per x plane
+    const size_t off = ((size_t)ia * h->nyh + h->h) * h->nz * es;
+    const size_t width = (size_t)h->ny * h->nz * es;
+    for (int n = mom ? 0 : 3; n < nf; ++n)
+      CU(cudaMemcpy2DAsync(hout[n] + off, plane_b, (char *)h->d_out[n] + off, plane_b, width,
+                           (size_t)(ib - ia), cudaMemcpyDeviceToHost, sout));
+    CU(cudaEventRecord(h->ev_d2h[c], sout));
+    return MONC_ADV_OK;
+  };
+  int rc;
+  if (h->overlap) {
+    for (int c = 0; c < C; ++c) {
+      if ((rc = h2d_chunk(c)) != MONC_ADV_OK) return rc;
+      if ((rc = compute_chunk(c)) != MONC_ADV_OK) return rc;
+      if ((rc = d2h_chunk(c)) != MONC_ADV_OK) return rc;
+    }
+  } else {
+    for (int c = 0; c < C; ++c) if ((rc = h2d_chunk(c)) != MONC_ADV_OK) return rc;
+    for (int c = 0; c < C; ++c) if ((rc = compute_chunk(c)) != MONC_ADV_OK) return rc;
+    for (int c = 0; c < C; ++c) if ((rc = d2h_chunk(c)) != MONC_ADV_OK) return rc;
+  }
+  if (user) CU(cudaStreamWaitEvent(user, h->ev_d2h[C - 1], 0));
+  h->in_flight = true;
+  h->have_times = false;
+  return MONC_ADV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int monc_adv_create(monc_adv_t *out, int nx, int ny, int nz, int halo, double dx, double dy,
+                    const double *dz, const double *dzn, const double *rho, const double *rhon,
+                    const double *tzc1, const double *tzc2, const double *tzd1,
+                    const double *tzd2, int dtype) {
+  if (!out) { g_create_error = "out is NULL"; return MONC_ADV_EINVAL; }
+  *out = nullptr;
+  auto bad = [&](const char *m) { g_create_error = m; return MONC_ADV_EINVAL; };
+  if (nx < 1 || ny < 1) return bad("nx, ny must be >= 1");
+  if (nz < 3) return bad("nz must be >= 3");
+  if (halo < 1) return bad("halo must be >= 1");
+  if (!(dx > 0) || !(dy > 0)) return bad("dx, dy must be > 0");
+  if (dtype != MONC_ADV_F64 && dtype != MONC_ADV_F32) return bad("dtype must be F64 or F32");
+  const int ntz = (tzc1 != nullptr) + (tzc2 != nullptr) + (tzd1 != nullptr) + (tzd2 != nullptr);
+  if (ntz != 0 && ntz != 4) return bad("tzc1, tzc2, tzd1, tzd2 must be all given or all NULL");
+  if (ntz == 0 && (!dz || !dzn || !rho || !rhon)) return bad("dz, dzn, rho, rhon required when tz arrays are NULL");
+  if ((long long)(nx + 2 * halo) * (ny + 2 * halo) * nz > (1LL << 40)) return bad("field too large");
+
+  monc_adv_s *h = new (std::nothrow) monc_adv_s;
+  if (!h) { g_create_error = "out of host memory"; return MONC_ADV_ENOMEM; }
+  h->nx = nx; h->ny = ny; h->nz = nz; h->h = halo; h->dtype = dtype;
+  h->nxh = nx + 2 * halo; h->nyh = ny + 2 * halo;
+  h->dx = dx; h->dy = dy;
+  h->elems = (size_t)h->nxh * h->nyh * nz;
+  h->esize = dtype == MONC_ADV_F64 ? 8 : 4;
+  auto cfail = [&](cudaError_t e, const char *what) {
+    g_create_error = std::string(what) + ": " + cudaGetErrorString(e);
+    const int code = e == cudaErrorMemoryAllocation ? MONC_ADV_ENOMEM : MONC_ADV_ECUDA;
+    for (void *p : h->d_tz) if (p) cudaFree(p);
+    delete h;
+    return code;
+  };
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e != cudaSuccess) return cfail(e, "cudaGetDevice");
+  e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
+  if (e != cudaSuccess) return cfail(e, "cudaDeviceGetAttribute");
+
+  // ---- coefficient tables (SURVEY.md 8(c).2 "Coefficients"), fp64 on the host
+  for (auto &t : h->tz_host) t.assign(nz, 0.0);
+  if (ntz == 4) {
+    const double *src[4] = {tzc1, tzc2, tzd1, tzd2};
+    for (int a = 0; a < 4; ++a) std::copy(src[a], src[a] + nz, h->tz_host[a].begin());
+  } else {
+    for (int k = 1; k <= nz - 1; ++k) {
+      const double den = 4.0 * rhon[k] * dz[k];
+      h->tz_host[0][k] = rho[k - 1] / den;
+      h->tz_host[1][k] = rho[k] / den;
+    }
+    for (int k = 1; k <= nz - 2; ++k) {
+      const double den = 4.0 * rho[k] * dzn[k + 1];
+      h->tz_host[2][k] = rhon[k] / den;
+      h->tz_host[3][k] = rhon[k + 1] / den;
+    }
+  }
+  // entries the definition never uses are pinned to 0 so the kernels need no
+  // special case: no tendency at K=1, no flux through the lid z_nz.
+  h->tz_host[0][0] = h->tz_host[1][0] = h->tz_host[2][0] = h->tz_host[3][0] = 0.0;
+  h->tz_host[1][nz - 1] = 0.0;
+  h->tz_host[2][nz - 1] = h->tz_host[3][nz - 1] = 0.0;
+  for (int a = 0; a < 4; ++a) {
+    e = cudaMalloc(&h->d_tz[a], (size_t)nz * h->esize);
+    if (e != cudaSuccess) return cfail(e, "cudaMalloc(constants)");
+    if (dtype == MONC_ADV_F64) {
+      e = cudaMemcpy(h->d_tz[a], h->tz_host[a].data(), (size_t)nz * 8, cudaMemcpyHostToDevice);
+    } else {
+      std::vector<float> f(nz);
+      for (int k = 0; k < nz; ++k) { f[k] = (float)h->tz_host[a][k]; h->tz_host[a][k] = (double)f[k]; }
+      e = cudaMemcpy(h->d_tz[a], f.data(), (size_t)nz * 4, cudaMemcpyHostToDevice);
+    }
+    if (e != cudaSuccess) return cfail(e, "cudaMemcpy(constants)");
+  }
+  g_create_error.clear();
+  *out = h;
+  return MONC_ADV_OK;
+}
+
+void monc_adv_destroy(monc_adv_t h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  if (h->in_flight) monc_adv_step_wait(h);
+  free_staging(h);
+  for (void *p : h->d_tz) if (p) cudaFree(p);
+  for (auto v : {&h->ev_h2d, &h->ev_kb, &h->ev_ke, &h->ev_d2h})
+    for (cudaEvent_t ev : *v) cudaEventDestroy(ev);
+  if (h->ev_user) cudaEventDestroy(h->ev_user);
+  if (h->ev_in_begin) cudaEventDestroy(h->ev_in_begin);
+  if (h->ev_out_begin) cudaEventDestroy(h->ev_out_begin);
+  if (h->s_in) cudaStreamDestroy(h->s_in);
+  if (h->s_k) cudaStreamDestroy(h->s_k);
+  if (h->s_out) cudaStreamDestroy(h->s_out);
+  delete h;
+}
+
+int monc_adv_bind_wind(monc_adv_t h, const void *u, const void *v, const void *w) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (!u || !v || !w) return fail(h, MONC_ADV_EINVAL, "bind_wind: NULL pointer");
+  if (!aligned16(u) || !aligned16(v) || !aligned16(w))
+    return fail(h, MONC_ADV_EINVAL, "bind_wind: pointers must be 16-byte aligned");
+  h->wind[0] = u; h->wind[1] = v; h->wind[2] = w;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_momentum(monc_adv_t h, const void *u, const void *v, const void *w, void *su,
+                      void *sv, void *sw, void *cuda_stream) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!u || !v || !w || !su || !sv || !sw) return fail(h, MONC_ADV_EINVAL, "momentum: NULL pointer");
+  const void *all[6] = {u, v, w, su, sv, sw};
+  for (const void *p : all)
+    if (!aligned16(p)) return fail(h, MONC_ADV_EINVAL, "momentum: pointers must be 16-byte aligned");
+  for (int a = 0; a < 3; ++a)
+    for (int b = 3; b < 6; ++b)
+      if (all[a] == all[b]) return fail(h, MONC_ADV_EINVAL, "momentum: inputs and outputs must not alias");
+  h->wind[0] = u; h->wind[1] = v; h->wind[2] = w;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->dtype == MONC_ADV_F64)
+    return launch_momentum<double>(h, (const double *)u, (const double *)v, (const double *)w,
+                                   (double *)su, (double *)sv, (double *)sw, h->h, h->h + h->nx, st);
+  return launch_momentum<float>(h, (const float *)u, (const float *)v, (const float *)w,
+                                (float *)su, (float *)sv, (float *)sw, h->h, h->h + h->nx, st);
+}
+
+int monc_adv_scalars(monc_adv_t h, const void *const *q, void *const *sq, int nq,
+                     void *cuda_stream) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (nq < 0 || nq > MONC_ADV_MAX_SCALARS) return fail(h, MONC_ADV_EINVAL, "scalars: nq out of range");
+  if (nq == 0) return MONC_ADV_OK;
+  if (!q || !sq) return fail(h, MONC_ADV_EINVAL, "scalars: NULL pointer table");
+  if (!h->wind[0]) return fail(h, MONC_ADV_ENOWIND, "scalars: no wind bound (call momentum or bind_wind first)");
+  for (int n = 0; n < nq; ++n) {
+    if (!q[n] || !sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: NULL field pointer");
+    if (!aligned16(q[n]) || !aligned16(sq[n]))
+      return fail(h, MONC_ADV_EINVAL, "scalars: pointers must be 16-byte aligned");
+    for (int m = 0; m < nq; ++m)
+      if (q[m] == sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: inputs and outputs must not alias");
+    for (int a = 0; a < 3; ++a)
+      if (h->wind[a] == sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: output aliases the wind");
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->dtype == MONC_ADV_F64)
+    return launch_scalars<double>(h, (const double *)h->wind[0], (const double *)h->wind[1],
+                                  (const double *)h->wind[2], q, sq, nq, h->h, h->h + h->nx, st);
+  return launch_scalars<float>(h, (const float *)h->wind[0], (const float *)h->wind[1],
+                               (const float *)h->wind[2], q, sq, nq, h->h, h->h + h->nx, st);
+}
+
+int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void *hw,
+                        const void *const *hq, int nq, void *hsu, void *hsv, void *hsw,
+                        void *const *hsq, void *cuda_stream) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "step_async: previous step still in flight (call step_wait)");
+  if (nq < 0 || nq > MONC_ADV_MAX_SCALARS) return fail(h, MONC_ADV_EINVAL, "step_async: nq out of range");
+  if (!hu || !hv || !hw) return fail(h, MONC_ADV_EINVAL, "step_async: NULL wind pointer");
+  const int nout = (hsu != nullptr) + (hsv != nullptr) + (hsw != nullptr);
+  if (nout != 0 && nout != 3) return fail(h, MONC_ADV_EINVAL, "step_async: hsu, hsv, hsw must be all given or all NULL");
+  if (nout == 0 && nq == 0) return fail(h, MONC_ADV_EINVAL, "step_async: nothing to compute");
+  if (nq > 0 && (!hq || !hsq)) return fail(h, MONC_ADV_EINVAL, "step_async: NULL pointer table");
+  for (int n = 0; n < nq; ++n)
+    if (!hq[n] || !hsq[n]) return fail(h, MONC_ADV_EINVAL, "step_async: NULL field pointer");
+  rc = ensure_async_objects(h, nq);
+  if (rc) return rc;
+  cudaStream_t user = (cudaStream_t)cuda_stream;
+  if (h->dtype == MONC_ADV_F64)
+    return step_async_impl<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
+  return step_async_impl<float>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
+}
+
+int monc_adv_step_inputs_consumed(monc_adv_t h) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!h->in_flight) return MONC_ADV_OK;
+  CU(cudaEventSynchronize(h->ev_h2d[h->chunk_a.size() - 1]));
+  return MONC_ADV_OK;
+}
+
+int monc_adv_step_wait_chunk(monc_adv_t h, int c) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!h->in_flight) return fail(h, MONC_ADV_EINVAL, "step_wait_chunk: no step in flight");
+  if (c < 0 || c >= (int)h->chunk_a.size()) return fail(h, MONC_ADV_EINVAL, "step_wait_chunk: chunk out of range");
+  CU(cudaEventSynchronize(h->ev_d2h[c]));
+  return MONC_ADV_OK;
+}
+
+int monc_adv_step_wait(monc_adv_t h) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!h->in_flight) return MONC_ADV_OK;
+  const int C = (int)h->chunk_a.size();
+  h->in_flight = false;
+  CU(cudaEventSynchronize(h->ev_d2h[C - 1]));
+  CU(cudaStreamSynchronize(h->s_in));
+  float t = 0, ksum = 0;
+  CU(cudaEventElapsedTime(&t, h->ev_in_begin, h->ev_h2d[C - 1]));
+  h->times[0] = t;
+  for (int c = 0; c < C; ++c) {
+    CU(cudaEventElapsedTime(&t, h->ev_kb[c], h->ev_ke[c]));
+    ksum += t;
+  }
+  h->times[1] = ksum;
+  CU(cudaEventElapsedTime(&t, h->ev_out_begin, h->ev_d2h[C - 1]));
+  h->times[2] = t;
+  CU(cudaEventElapsedTime(&t, h->ev_in_begin, h->ev_d2h[C - 1]));
+  h->times[3] = t;
+  h->have_times = true;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_step_chunk_range(monc_adv_t h, int c, int *x_begin, int *x_end) {
+  if (!h) return MONC_ADV_EINVAL;
+  const int C = std::min(h->nchunks, h->nx);
+  if (c < 0 || c >= C || !x_begin || !x_end) return fail(h, MONC_ADV_EINVAL, "step_chunk_range: bad argument");
+  *x_begin = (int)((long long)h->nx * c / C);
+  *x_end = (int)((long long)h->nx * (c + 1) / C);
+  return MONC_ADV_OK;
+}
+
+int monc_adv_step_times_ms(monc_adv_t h, float out[4]) {
+  if (!h || !out) return MONC_ADV_EINVAL;
+  if (!h->have_times) return fail(h, MONC_ADV_EINVAL, "step_times_ms: no completed step");
+  for (int a = 0; a < 4; ++a) out[a] = h->times[a];
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_chunks(monc_adv_t h, int nchunks) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_chunks: step in flight");
+  if (nchunks < 1 || nchunks > h->nx) return fail(h, MONC_ADV_EINVAL, "set_chunks: need 1 <= nchunks <= nx");
+  h->nchunks = nchunks;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_overlap(monc_adv_t h, int on) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_overlap: step in flight");
+  h->overlap = on ? 1 : 0;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_form(monc_adv_t h, int form) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (form != MONC_ADV_FORM_FLUX && form != MONC_ADV_FORM_PW_SKEW)
+    return fail(h, MONC_ADV_EINVAL, "set_form: unknown form");
+  h->form = form;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_accumulate(monc_adv_t h, int on) {
+  if (!h) return MONC_ADV_EINVAL;
+  h->accumulate = on ? 1 : 0;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_variant(monc_adv_t h, int variant) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (variant < 0 || variant > 2) return fail(h, MONC_ADV_EINVAL, "set_variant: 0, 1 or 2");
+  if (variant == 2) {
+    const int nk = h->dtype == MONC_ADV_F64 ? 2 : 4;
+    if (h->nz % nk != 0) return fail(h, MONC_ADV_EINVAL, "set_variant: marching kernels need nz % (16/sizeof(dtype)) == 0");
+  }
+  h->variant = variant;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (xchunk < 0 || group < 0) return fail(h, MONC_ADV_EINVAL, "set_tuning: negative value");
+  h->xchunk = xchunk;
+  h->group = group;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_get_coefficients(monc_adv_t h, double *tzc1, double *tzc2, double *tzd1,
+                              double *tzd2) {
+  if (!h) return MONC_ADV_EINVAL;
+  double *dst[4] = {tzc1, tzc2, tzd1, tzd2};
+  for (int a = 0; a < 4; ++a)
+    if (dst[a]) std::copy(h->tz_host[a].begin(), h->tz_host[a].end(), dst[a]);
+  return MONC_ADV_OK;
+}
+
+long monc_adv_launch_count(monc_adv_t h) { return h ? h->launches : 0; }
+
+const char *monc_adv_last_error(monc_adv_t h) {
+  return h ? h->err.c_str() : g_create_error.c_str();
+}
+
+const char *monc_adv_version(void) { return "monc-adv-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,411 @@
+// monc_adv_kernels.cuh -- sm_100a kernels for MONC's advection source terms.
+//
+// Definition implemented: SURVEY.md 8(c).2 / DESIGN.md "Definition" (flux-form
+// centred advection on the Arakawa C grid, z-fastest layout).  The paper
+// runs "the advection kernel ... for the entirety of the field
+// (each column at the same time)"; these kernels are that step, re-designed
+// for B200: an HBM-bound stencil, so the design goal is algorithmic DRAM
+// traffic (every input read once, every output written once) with enough
+// bytes in flight, not flops.  No tensor cores: there is no dense contraction.
+//
+// Two families:
+//   generic_*  one thread per output point, direct loads.  Always valid (any
+//              nz, both forms); the fallback and the "naive" baseline.
+//   march_*    the fast path.  lane <-> z (16-byte vectors, coalesced along
+//              MONC's fastest axis), warp <-> (column j, 32-vector z chunk),
+//              block marches a chunk of x planes.  Values that an x-neighbour
+//              step needs again stay in registers (raw E-plane values and the
+//              three x-face fluxes), vertical neighbours come from warp
+//              shuffles, y neighbours from L1 (adjacent warps load the same
+//              lines).  Every face flux is computed once per thread: the
+//              nine flux differences of the momentum equations need only six
+//              distinct products because the off-diagonal ones are shared
+//              (FxV == FyU, FxW == FzU, FyW == FzV).
+//
+// This header shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace monc {
+
+constexpr int kMaxScalars = 64;
+constexpr int kWarpsPerBlock = 8;
+
+template <typename T>
+struct KParams {
+  int nx, ny, nz, h;
+  int nyh;          // ny + 2h
+  long long plane;  // nyh * nz elements
+  int ia, ib;       // output x range [ia, ib), array indices
+  int xc;           // x planes marched per block
+  int wzc;          // warps (z chunks of 32 vectors) per column
+  int units;        // ny * wzc
+  int accumulate;   // 0: overwrite, 1: add into outputs
+  int skew;         // generic kernels only: PW skew form
+  T cx, cy;         // 1/(4dx), 1/(4dy)
+  const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz; tzc2[nz-1] = 0
+};
+
+template <typename T>
+struct ScalarPtrs {
+  const T *q[kMaxScalars];
+  T *sq[kMaxScalars];
+};
+
+// ---------------------------------------------------------------------------
+// 16-byte vectors along z
+// ---------------------------------------------------------------------------
+template <typename T> struct VecOf;
+template <> struct VecOf<double> { static constexpr int NK = 2; };
+template <> struct VecOf<float> { static constexpr int NK = 4; };
+
+template <typename T>
+struct Vec {
+  T v[VecOf<T>::NK];
+};
+
+__device__ __forceinline__ Vec<double> ld_vec(const double *p) {
+  const double2 t = __ldg(reinterpret_cast<const double2 *>(p));
+  Vec<double> r;
+  r.v[0] = t.x; r.v[1] = t.y;
+  return r;
+}
+__device__ __forceinline__ Vec<float> ld_vec(const float *p) {
+  const float4 t = __ldg(reinterpret_cast<const float4 *>(p));
+  Vec<float> r;
+  r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+  return r;
+}
+__device__ __forceinline__ Vec<double> ld_vec_rw(const double *p) {
+  const double2 t = *reinterpret_cast<const double2 *>(p);
+  Vec<double> r;
+  r.v[0] = t.x; r.v[1] = t.y;
+  return r;
+}
+__device__ __forceinline__ Vec<float> ld_vec_rw(const float *p) {
+  const float4 t = *reinterpret_cast<const float4 *>(p);
+  Vec<float> r;
+  r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+  return r;
+}
+// streaming (evict-first) stores: tendencies are never re-read by the kernel
+__device__ __forceinline__ void st_vec(double *p, const Vec<double> &a) {
+  __stcs(reinterpret_cast<double2 *>(p), make_double2(a.v[0], a.v[1]));
+}
+__device__ __forceinline__ void st_vec(float *p, const Vec<float> &a) {
+  __stcs(reinterpret_cast<float4 *>(p), make_float4(a.v[0], a.v[1], a.v[2], a.v[3]));
+}
+
+template <typename T>
+__device__ __forceinline__ Vec<T> ld_or_zero(const T *p, bool act) {
+  Vec<T> r;
+#pragma unroll
+  for (int e = 0; e < VecOf<T>::NK; ++e) r.v[e] = T(0);
+  if (act) r = ld_vec(p);
+  return r;
+}
+
+constexpr unsigned kFull = 0xffffffffu;
+
+// value one level above each element: r[e] = a[e+1]; the last comes from the
+// next lane's first element, or (warp's last lane) from `edge`.
+template <typename T>
+__device__ __forceinline__ Vec<T> shift_up(const Vec<T> &a, int lane, T edge) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> r;
+#pragma unroll
+  for (int e = 0; e + 1 < NK; ++e) r.v[e] = a.v[e + 1];
+  T nxt = __shfl_down_sync(kFull, a.v[0], 1);
+  r.v[NK - 1] = (lane == 31) ? edge : nxt;
+  return r;
+}
+// flux one level below each element: r[e] = f[e-1]; the first comes from the
+// previous lane's last element, or (warp's first lane) from `edge`.
+template <typename T>
+__device__ __forceinline__ Vec<T> shift_down(const Vec<T> &f, int lane, T edge) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> r;
+#pragma unroll
+  for (int e = 1; e < NK; ++e) r.v[e] = f.v[e - 1];
+  T prv = __shfl_up_sync(kFull, f.v[NK - 1], 1);
+  r.v[0] = (lane == 0) ? edge : prv;
+  return r;
+}
+
+// ---------------------------------------------------------------------------
+// march_momentum: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks su/sv/sw)
+// ---------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict__ v,
+               const T *__restrict__ w, T *__restrict__ su, T *__restrict__ sv,
+               T *__restrict__ sw) {
+  constexpr int NK = VecOf<T>::NK;
+  const int lane = threadIdx.x & 31;
+  const int unit = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  if (unit >= p.units) return;  // warp-uniform
+  const int jr = unit / p.wzc;
+  const int zc = unit - jr * p.wzc;
+  const int k0 = (zc * 32 + lane) * NK;
+  const bool act = k0 < p.nz;
+  const bool top_edge = act && lane == 31 && (k0 + NK < p.nz);
+  const bool bot_edge = act && lane == 0 && zc > 0;
+  const int i0 = p.ia + blockIdx.y * p.xc;
+  const int i1 = min(p.ib, i0 + p.xc);
+  const long long nz = p.nz, plane = p.plane;
+
+  // per-level coefficients, kept in registers for the whole march
+  Vec<T> c1 = ld_or_zero(p.tzc1 + k0, act), c2 = ld_or_zero(p.tzc2 + k0, act);
+  Vec<T> d1 = ld_or_zero(p.tzd1 + k0, act), d2 = ld_or_zero(p.tzd2 + k0, act);
+  const T cx = p.cx, cy = p.cy;
+
+  long long c = ((long long)(i0 - 1) * p.nyh + (jr + p.h)) * nz + k0;  // (i, j, k0)
+  // values of the centre plane that the previous step already loaded
+  Vec<T> uC = ld_or_zero(u + c, act), vC = ld_or_zero(v + c, act);
+  Vec<T> vS = ld_or_zero(v + c - nz, act), wC = ld_or_zero(w + c, act);
+  // x-face fluxes on the west side, carried from the previous step
+  Vec<T> fxx_w, fxy_w, fxz_w;
+#pragma unroll
+  for (int e = 0; e < NK; ++e) fxx_w.v[e] = fxy_w.v[e] = fxz_w.v[e] = T(0);
+
+#pragma unroll 1
+  for (int i = i0 - 1; i < i1; ++i, c += plane) {
+    const Vec<T> uS = ld_or_zero(u + c - nz, act), uN = ld_or_zero(u + c + nz, act);
+    const Vec<T> vN = ld_or_zero(v + c + nz, act);
+    const Vec<T> wS = ld_or_zero(w + c - nz, act), wN = ld_or_zero(w + c + nz, act);
+    const Vec<T> uE = ld_or_zero(u + c + plane, act), vE = ld_or_zero(v + c + plane, act);
+    const Vec<T> vSE = ld_or_zero(v + c + plane - nz, act), wE = ld_or_zero(w + c + plane, act);
+    // z-chunk edges: one lane each reads the few scalars a shuffle cannot give
+    T e_u = T(0), e_v = T(0), e_w = T(0), e_vs = T(0);
+    if (top_edge) {
+      e_u = __ldg(u + c + NK); e_v = __ldg(v + c + NK);
+      e_w = __ldg(w + c + NK); e_vs = __ldg(v + c - nz + NK);
+    }
+    T b_xz = T(0), b_yz = T(0), b_zz = T(0);
+    if (bot_edge) {
+      const T ub = __ldg(u + c - 1), vb = __ldg(v + c - 1), wb = __ldg(w + c - 1);
+      const T web = __ldg(w + c + plane - 1), wnb = __ldg(w + c + nz - 1);
+      b_xz = (ub + uC.v[0]) * (wb + web);
+      b_yz = (vb + vC.v[0]) * (wb + wnb);
+      b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+    }
+    const Vec<T> uCu = shift_up(uC, lane, e_u), vCu = shift_up(vC, lane, e_v);
+    const Vec<T> wCu = shift_up(wC, lane, e_w), vSu = shift_up(vS, lane, e_vs);
+
+    Vec<T> fxx_e, fxy_e, fxz_e, fyz_n, fzz_t, ry, rv, rwy;
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      const T a = uC.v[e] + uE.v[e];
+      fxx_e.v[e] = a * a;                                              // (u_i+u_i+1)^2
+      fxy_e.v[e] = (uC.v[e] + uN.v[e]) * (vC.v[e] + vE.v[e]);          // corner (i+1/2, j+1/2)
+      const T fxy_se = (uS.v[e] + uC.v[e]) * (vS.v[e] + vSE.v[e]);     // corner (i+1/2, j-1/2)
+      fxz_e.v[e] = (uC.v[e] + uCu.v[e]) * (wC.v[e] + wE.v[e]);         // (i+1/2, z_K)
+      const T bn = vC.v[e] + vN.v[e], bs = vS.v[e] + vC.v[e];
+      fyz_n.v[e] = (vC.v[e] + vCu.v[e]) * (wC.v[e] + wN.v[e]);         // (j+1/2, z_K)
+      const T fyz_s = (vS.v[e] + vSu.v[e]) * (wS.v[e] + wC.v[e]);      // (j-1/2, z_K)
+      const T g = wC.v[e] + wCu.v[e];
+      fzz_t.v[e] = g * g;                                              // at zn_{K+1}
+      // horizontal parts
+      ry.v[e] = cy * (fxy_se - fxy_e.v[e]);                            // su: y
+      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);                            // sw: y
+      rv.v[e] = cx * (fxy_w.v[e] - fxy_e.v[e]) + cy * (bs * bs - bn * bn);  // sv: x + y
+    }
+    const Vec<T> fxz_b = shift_down(fxz_e, lane, b_xz);
+    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
+    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
+
+    if (i >= i0 && act) {
+      Vec<T> ou, ov, ow;
+#pragma unroll
+      for (int e = 0; e < NK; ++e) {
+        const int k = k0 + e;
+        T xu = cx * (fxx_w.v[e] - fxx_e.v[e]) + ry.v[e] +
+               (c1.v[e] * fxz_b.v[e] - c2.v[e] * fxz_e.v[e]);
+        T xv = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
+        T xw = cx * (fxz_w.v[e] - fxz_e.v[e]) + rwy.v[e] +
+               (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+        if (k == 0) { xu = T(0); xv = T(0); xw = T(0); }
+        if (k == p.nz - 1) xw = T(0);
+        ou.v[e] = xu; ov.v[e] = xv; ow.v[e] = xw;
+      }
+      if (p.accumulate) {
+        const Vec<T> au = ld_vec_rw(su + c), av = ld_vec_rw(sv + c), aw = ld_vec_rw(sw + c);
+#pragma unroll
+        for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
+      }
+      st_vec(su + c, ou); st_vec(sv + c, ov); st_vec(sw + c, ow);
+    }
+    // rotate: east becomes centre
+    fxx_w = fxx_e; fxy_w = fxy_e; fxz_w = fxz_e;
+    uC = uE; vC = vE; vS = vSE; wC = wE;
+  }
+}
+
+// ---------------------------------------------------------------------------
+// march_scalars<G>: G scalars per thread share one read of the wind
+// (SURVEY.md 8(a) row a2, 8(c).2 block sq; PAPER.md:83 wind shared by kernels)
+// ---------------------------------------------------------------------------
+template <typename T, int G>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+march_scalars(const KParams<T> p, const ScalarPtrs<T> ptrs, const int nq, const int ngroups,
+              const T *__restrict__ u, const T *__restrict__ v, const T *__restrict__ w) {
+  constexpr int NK = VecOf<T>::NK;
+  const int lane = threadIdx.x & 31;
+  const int grp = blockIdx.x % ngroups;  // group index fastest: co-scheduled blocks share the wind in L2
+  const int unit = (blockIdx.x / ngroups) * kWarpsPerBlock + (threadIdx.x >> 5);
+  if (unit >= p.units) return;
+  const int s0 = grp * G;
+  const int cnt = min(G, nq - s0);
+  const int jr = unit / p.wzc;
+  const int zc = unit - jr * p.wzc;
+  const int k0 = (zc * 32 + lane) * NK;
+  const bool act = k0 < p.nz;
+  const bool top_edge = act && lane == 31 && (k0 + NK < p.nz);
+  const bool bot_edge = act && lane == 0 && zc > 0;
+  const int i0 = p.ia + blockIdx.y * p.xc;
+  const int i1 = min(p.ib, i0 + p.xc);
+  const long long nz = p.nz, plane = p.plane;
+
+  Vec<T> c1 = ld_or_zero(p.tzc1 + k0, act), c2 = ld_or_zero(p.tzc2 + k0, act);
+#pragma unroll
+  for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
+  const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
+
+  long long c = ((long long)(i0 - 1) * p.nyh + (jr + p.h)) * nz + k0;
+  Vec<T> qC[G], fx_w[G];
+#pragma unroll
+  for (int s = 0; s < G; ++s) {
+    qC[s] = ld_or_zero(ptrs.q[s0 + (s < cnt ? s : 0)] + c, act);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) fx_w[s].v[e] = T(0);
+  }
+
+#pragma unroll 1
+  for (int i = i0 - 1; i < i1; ++i, c += plane) {
+    const Vec<T> uC = ld_or_zero(u + c, act), vC = ld_or_zero(v + c, act);
+    const Vec<T> vS = ld_or_zero(v + c - nz, act), wC = ld_or_zero(w + c, act);
+    const T wb = bot_edge ? __ldg(w + c - 1) : T(0);
+#pragma unroll
+    for (int s = 0; s < G; ++s) {
+      if (s < cnt) {  // block-uniform
+        const T *__restrict__ q = ptrs.q[s0 + s];
+        const Vec<T> qE = ld_or_zero(q + c + plane, act);
+        const Vec<T> qS = ld_or_zero(q + c - nz, act), qN = ld_or_zero(q + c + nz, act);
+        const T e_q = top_edge ? __ldg(q + c + NK) : T(0);
+        const T b_z = bot_edge ? wb * (__ldg(q + c - 1) + qC[s].v[0]) : T(0);
+        const Vec<T> qCu = shift_up(qC[s], lane, e_q);
+        Vec<T> fz_t, fx_e, hy;
+#pragma unroll
+        for (int e = 0; e < NK; ++e) {
+          fx_e.v[e] = uC.v[e] * (qC[s].v[e] + qE.v[e]);
+          hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + qC[s].v[e]) - vC.v[e] * (qC[s].v[e] + qN.v[e]));
+          fz_t.v[e] = wC.v[e] * (qC[s].v[e] + qCu.v[e]);
+        }
+        const Vec<T> fz_b = shift_down(fz_t, lane, b_z);
+        if (i >= i0 && act) {
+          T *sq = ptrs.sq[s0 + s];
+          Vec<T> o;
+#pragma unroll
+          for (int e = 0; e < NK; ++e) {
+            T x = cx2 * (fx_w[s].v[e] - fx_e.v[e]) + hy.v[e] +
+                  (c1.v[e] * fz_b.v[e] - c2.v[e] * fz_t.v[e]);
+            if (k0 + e == 0) x = T(0);
+            o.v[e] = x;
+          }
+          if (p.accumulate) {
+            const Vec<T> a = ld_vec_rw(sq + c);
+#pragma unroll
+            for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
+          }
+          st_vec(sq + c, o);
+        }
+        fx_w[s] = fx_e;
+        qC[s] = qE;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// generic kernels: one thread per interior point, formulas as written
+// ---------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+generic_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict__ v,
+                 const T *__restrict__ w, T *__restrict__ su, T *__restrict__ sv,
+                 T *__restrict__ sw) {
+  const long long n = (long long)(p.ib - p.ia) * p.ny * p.nz;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const int k = (int)(t % p.nz);
+  const long long r = t / p.nz;
+  const int j = (int)(r % p.ny) + p.h;
+  const int i = (int)(r / p.ny) + p.ia;
+  const long long nz = p.nz, pl = p.plane;
+  const long long c = ((long long)i * p.nyh + j) * nz + k;
+  T xu = T(0), xv = T(0), xw = T(0);
+  if (k > 0) {
+    const T uc = u[c], vc = v[c], wc = w[c];
+    const T ua = p.skew ? T(0) : uc, va = p.skew ? T(0) : vc, wa = p.skew ? T(0) : wc;
+    const bool top = (k == p.nz - 1);
+    const T c1 = p.tzc1[k], c2 = p.tzc2[k];
+    {
+      const T X = p.cx * ((u[c - pl] + uc) * (u[c - pl] + ua) - (uc + u[c + pl]) * (ua + u[c + pl]));
+      const T Y = p.cy * ((v[c - nz] + v[c + pl - nz]) * (u[c - nz] + ua) -
+                          (vc + v[c + pl]) * (ua + u[c + nz]));
+      T Z = c1 * (w[c - 1] + w[c + pl - 1]) * (u[c - 1] + ua);
+      if (!top) Z -= c2 * (wc + w[c + pl]) * (ua + u[c + 1]);
+      xu = X + Y + Z;
+    }
+    {
+      const T Y = p.cy * ((v[c - nz] + vc) * (v[c - nz] + va) - (vc + v[c + nz]) * (va + v[c + nz]));
+      const T X = p.cx * ((u[c - pl] + u[c - pl + nz]) * (v[c - pl] + va) -
+                          (uc + u[c + nz]) * (va + v[c + pl]));
+      T Z = c1 * (w[c - 1] + w[c + nz - 1]) * (v[c - 1] + va);
+      if (!top) Z -= c2 * (wc + w[c + nz]) * (va + v[c + 1]);
+      xv = Y + X + Z;
+    }
+    if (!top) {
+      const T X = p.cx * ((u[c - pl] + u[c - pl + 1]) * (w[c - pl] + wa) -
+                          (uc + u[c + 1]) * (wa + w[c + pl]));
+      const T Y = p.cy * ((v[c - nz] + v[c - nz + 1]) * (w[c - nz] + wa) -
+                          (vc + v[c + 1]) * (wa + w[c + nz]));
+      const T Z = p.tzd1[k] * (w[c - 1] + wc) * (w[c - 1] + wa) -
+                  p.tzd2[k] * (wc + w[c + 1]) * (wa + w[c + 1]);
+      xw = X + Y + Z;
+    }
+  }
+  if (p.accumulate) { xu += su[c]; xv += sv[c]; xw += sw[c]; }
+  su[c] = xu; sv[c] = xv; sw[c] = xw;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+generic_scalars(const KParams<T> p, const ScalarPtrs<T> ptrs, const T *__restrict__ u,
+                const T *__restrict__ v, const T *__restrict__ w) {
+  const long long n = (long long)(p.ib - p.ia) * p.ny * p.nz;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const T *__restrict__ q = ptrs.q[blockIdx.y];
+  T *__restrict__ sq = ptrs.sq[blockIdx.y];
+  const int k = (int)(t % p.nz);
+  const long long r = t / p.nz;
+  const int j = (int)(r % p.ny) + p.h;
+  const int i = (int)(r / p.ny) + p.ia;
+  const long long nz = p.nz, pl = p.plane;
+  const long long c = ((long long)i * p.nyh + j) * nz + k;
+  T x = T(0);
+  if (k > 0) {
+    const T qc = q[c];
+    const T qa = p.skew ? T(0) : qc;
+    const T X = T(2) * p.cx * (u[c - pl] * (q[c - pl] + qa) - u[c] * (qa + q[c + pl]));
+    const T Y = T(2) * p.cy * (v[c - nz] * (q[c - nz] + qa) - v[c] * (qa + q[c + nz]));
+    T Z = T(2) * p.tzc1[k] * w[c - 1] * (q[c - 1] + qa);
+    if (k < p.nz - 1) Z -= T(2) * p.tzc2[k] * w[c] * (qa + q[c + 1]);
+    x = X + Y + Z;
+  }
+  if (p.accumulate) x += sq[c];
+  sq[c] = x;
+}
+
+}  // namespace monc

@@ -1,0 +1,290 @@
+"""GPU parity: the CUDA library (through the C ABI) against the CPU oracle on
+the same seeded inputs, element by element.  Run on the B200 box: -m gpu."""
+import dataclasses
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2009_12850_b200 import binding, synth
+import gpu_common as gc
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu(gpu_required):
+    yield
+    torch.cuda.synchronize()
+
+
+def run_momentum(cfg, variant="auto", xchunk=0, fields=None, form="flux"):
+    P, L = gc.make_pair(cfg)
+    L.set_variant(variant)
+    L.set_tuning(xchunk=xchunk)
+    L.set_form(form)
+    U, V, W = fields if fields is not None else [synth.field(cfg, n) for n in "uvw"]
+    want = P.momentum(U, V, W, skew=(form == "pw_skew"), nthreads=oracle.max_threads())
+    du, dv, dw = (gc.to_dev(a, L) for a in (U, V, W))
+    outs = gc.fresh_out(L, 3)
+    L.momentum(du, dv, dw, *outs)
+    torch.cuda.synchronize()
+    errs = [gc.check(cfg, o, w_, n) for o, w_, n in zip(outs, want, ("su", "sv", "sw"))]
+    for o, n in zip(outs, ("su", "sv", "sw")):
+        gc.check_halo_untouched(cfg, o, n)
+    L.close()
+    return errs
+
+
+def run_scalars(cfg, nq, variant="auto", xchunk=0, group=0, form="flux"):
+    cfgq = dataclasses.replace(cfg, nq=nq)
+    P, L = gc.make_pair(cfgq)
+    L.set_variant(variant)
+    L.set_tuning(xchunk=xchunk, group=group)
+    L.set_form(form)
+    U, V, W = [synth.field(cfgq, n) for n in "uvw"]
+    names = synth.field_names(cfgq)
+    Q = [synth.field(cfgq, n) for n in names]
+    du, dv, dw = (gc.to_dev(a, L) for a in (U, V, W))
+    dq = [gc.to_dev(a, L) for a in Q]
+    outs = gc.fresh_out(L, nq)
+    L.bind_wind(du, dv, dw)
+    L.scalars(dq, outs)
+    torch.cuda.synchronize()
+    for n, (o, q) in enumerate(zip(outs, Q)):
+        want = P.scalar(U, V, W, q, skew=(form == "pw_skew"), nthreads=oracle.max_threads())
+        gc.check(cfgq, o, want, f"sq[{names[n]}]")
+        gc.check_halo_untouched(cfgq, o, names[n])
+    L.close()
+
+
+# ---------------------------------------------------------------------------
+# BASELINE.json configs 0 and 1: full element-by-element comparison
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["march", "generic"])
+def test_config0_momentum_fp64(variant):
+    run_momentum(synth.CONFIGS[0], variant)
+
+
+@pytest.mark.parametrize("variant", ["march", "generic"])
+def test_config0_scalars_fp64(variant):
+    run_scalars(synth.CONFIGS[0], 4, variant)
+
+
+def test_config1_momentum_fp64_full_size():
+    # the launch configuration bench.py times (variant auto, default tuning)
+    errs = run_momentum(synth.CONFIGS[1])
+    print("config1 max rel errs", errs)
+
+
+def test_config1_shape_fp32_and_scalars():
+    cfg = dataclasses.replace(synth.CONFIGS[1], dtype="f32")
+    run_momentum(cfg)
+    run_scalars(dataclasses.replace(synth.CONFIGS[1], nx=64), 3)
+
+
+# ---------------------------------------------------------------------------
+# ragged / edge shapes: several tiles, partial warps, z-chunk edges, odd sizes
+# ---------------------------------------------------------------------------
+SHAPES = [
+    (13, 7, 38, 2),    # fp64 vectors ok, fp32 falls back to generic (38 % 4 != 0)
+    (9, 11, 37, 2),    # odd nz: generic kernels
+    (10, 6, 70, 2),    # two z-chunks per column, ragged second chunk
+    (6, 10, 160, 2),   # config 4's nz: 2.5 warps per column (fp64)
+    (5, 9, 256, 1),    # halo 1, 4 z-chunks per column (fp64), 2 (fp32)
+    (7, 5, 64, 3),     # halo 3, exactly one full warp per column (fp64)
+    (3, 1, 4, 2),      # ny = 1
+    (1, 3, 3, 2),      # nx = 1, minimum nz
+    (33, 17, 132, 2),  # > 1 chunk in every direction
+]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_ragged_shapes(shape, dtype):
+    nx, ny, nz, h = shape
+    cfg = gc.custom_cfg(nx, ny, nz, halo=h, dtype=dtype, cid=200 + nz)
+    run_momentum(cfg, "auto", xchunk=0)
+    run_momentum(cfg, "auto", xchunk=4)   # several x-chunks: chunk seams
+    run_scalars(cfg, 3, "auto", xchunk=5, group=2)   # ragged group (2 + 1)
+
+
+@pytest.mark.parametrize("group", [1, 2, 3, 4, 5])
+def test_scalar_group_sizes(group):
+    cfg = gc.custom_cfg(12, 9, 70, nq=7, cid=300)
+    run_scalars(cfg, 7, "march", xchunk=5, group=group)
+
+
+def test_max_scalars_and_zero():
+    cfg = gc.custom_cfg(4, 4, 8, cid=301)
+    P, L = gc.make_pair(cfg)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    du, dv, dw = (gc.to_dev(a, L) for a in (U, V, W))
+    L.bind_wind(du, dv, dw)
+    L.scalars([], [])  # nq = 0: no-op
+    cfgq = dataclasses.replace(cfg, nq=binding.MAX_SCALARS)
+    names = synth.field_names(cfgq)
+    Q = [synth.field(cfgq, n) for n in names]
+    dq = [gc.to_dev(a, L) for a in Q]
+    outs = gc.fresh_out(L, len(Q))
+    L.scalars(dq, outs)
+    torch.cuda.synchronize()
+    for o, q in zip(outs, Q):
+        gc.check(cfg, o, P.scalar(U, V, W, q), "sq")
+    with pytest.raises(binding.MoncAdvError) as e:
+        L.scalars(dq + [dq[0]], outs + gc.fresh_out(L, 1))
+    assert e.value.code == binding.EINVAL
+
+
+# ---------------------------------------------------------------------------
+# P7 worked example through the library: exact in fp64 AND fp32
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("variant", ["march", "generic"])
+def test_P7_exact_through_gpu(dtype, variant):
+    from test_oracle_pins import p7_problem, read_golden
+    P, (U, V, W, Q) = p7_problem()
+    dz = np.array([1, 1, 2, 2, 4, 4], float)
+    L = binding.MoncAdv(4, 4, 6, 2, 2.0, 4.0, dz, dz, np.array([1, 1, .5, .5, .25, .25]),
+                        np.array([2, 1, 1, .5, .5, .25]), dtype=dtype)
+    if variant == "march" and dtype == "f32":
+        with pytest.raises(binding.MoncAdvError):
+            L.set_variant("march")  # nz = 6 is not a multiple of 4
+        return
+    L.set_variant(variant)
+    # coefficient tables as the library stores them
+    tz = dict(zip(("tzc1", "tzc2", "tzd1", "tzd2"), L.get_coefficients()))
+    d = [gc.to_dev(a, L) for a in (U, V, W, Q)]
+    outs = gc.fresh_out(L, 4)
+    L.momentum(d[0], d[1], d[2], *outs[:3])
+    L.scalars([d[3]], [outs[3]])
+    torch.cuda.synchronize()
+    res = {k: o.cpu().numpy().astype(np.float64)[2:6, 2:6] for k, o in zip(("su", "sv", "sw", "sq"), outs)}
+    pos = np.arange(1, 97, dtype=float).reshape(4, 4, 6)
+    n = 0
+    for r in read_golden():
+        if r[0] == "coef" and r[1] in tz:
+            vals = [float(Fraction(x)) for x in r[2:]]
+            if r[1] == "tzc2":
+                vals[-1] = 0.0  # the library pins the unused lid entry to 0
+            assert list(tz[r[1]]) == vals
+        if r[0] == "column" and r[1] == "flux":
+            vals = [float(Fraction(x)) for x in r[5:]]
+            assert list(res[r[2]][int(r[3]), int(r[4])]) == vals, (r[2], r[3], r[4])
+            n += 1
+        if r[0] == "checksum":
+            s, sa, mx, sidx = (float(Fraction(x)) for x in r[3:])
+            a = res[r[2]]
+            assert a.sum() == s and np.abs(a).sum() == sa and np.abs(a).max() == mx
+            assert (a * pos).sum() == sidx
+            n += 1
+    assert n == 16
+    # and every point equals the oracle bitwise (all values exactly representable)
+    want = list(P.momentum(U, V, W)) + [P.scalar(U, V, W, Q)]
+    for k, w_ in zip(("su", "sv", "sw", "sq"), want):
+        assert np.array_equal(res[k], w_[2:6, 2:6]), k
+    L.close()
+
+
+# ---------------------------------------------------------------------------
+# semantics: accumulate, wind binding, skew form, errors
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["march", "generic"])
+def test_accumulate_mode(variant):
+    cfg = gc.custom_cfg(9, 8, 66, nq=2, cid=302)
+    P, L = gc.make_pair(cfg)
+    L.set_variant(variant)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    Q = [synth.field(cfg, n) for n in synth.field_names(cfg)]
+    d = [gc.to_dev(a, L) for a in (U, V, W)]
+    dq = [gc.to_dev(a, L) for a in Q]
+    base = [torch.randn(L.shape, device="cuda", dtype=torch.float64) for _ in range(5)]
+    outs = [b.clone() for b in base]
+    L.set_accumulate(True)
+    L.momentum(*d, *outs[:3])
+    L.scalars(dq, outs[3:])
+    L.set_accumulate(False)
+    plain = gc.fresh_out(L, 5)
+    L.momentum(*d, *plain[:3])
+    L.scalars(dq, plain[3:])
+    torch.cuda.synchronize()
+    h = cfg.halo
+    for b, o, p_ in zip(base, outs, plain):
+        sl = (slice(h, h + cfg.nx), slice(h, h + cfg.ny))
+        # additivity: bitwise equal to a separate add
+        assert torch.equal(o[sl], b[sl] + p_[sl])
+        m = torch.ones(L.shape, dtype=torch.bool, device="cuda")
+        m[sl] = False
+        assert torch.equal(o[m], b[m])  # halos untouched
+    L.close()
+
+
+def test_scalars_need_wind_and_wind_binding_equivalence():
+    cfg = gc.custom_cfg(8, 8, 32, nq=2, cid=303)
+    P, L = gc.make_pair(cfg)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    Q = [synth.field(cfg, n) for n in synth.field_names(cfg)]
+    d = [gc.to_dev(a, L) for a in (U, V, W)]
+    dq = [gc.to_dev(a, L) for a in Q]
+    o1, o2 = gc.fresh_out(L, 2), gc.fresh_out(L, 2)
+    with pytest.raises(binding.MoncAdvError) as e:
+        L.scalars(dq, o1)
+    assert e.value.code == binding.ENOWIND
+    L.bind_wind(*d)
+    L.scalars(dq, o1)
+    L.momentum(*d, *gc.fresh_out(L, 3))   # binds the same wind
+    L.scalars(dq, o2)
+    torch.cuda.synchronize()
+    for a, b in zip(o1, o2):
+        assert torch.equal(a, b)
+    # aliasing is refused
+    with pytest.raises(binding.MoncAdvError):
+        L.momentum(d[0], d[1], d[2], d[0], o1[0], o1[1])
+    L.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_pw_skew_form(dtype):
+    cfg = gc.custom_cfg(10, 9, 40, dtype=dtype, cid=304)
+    run_momentum(cfg, form="pw_skew")
+    run_scalars(cfg, 2, form="pw_skew")
+
+
+def test_translation_invariance_bitwise_on_gpu():
+    # P10 through the library: no dependence on absolute position or block seams
+    cfg = gc.custom_cfg(16, 12, 64, cid=305)
+    P, L = gc.make_pair(cfg)
+    L.set_tuning(xchunk=5)
+    fs = [synth.interior_field(cfg, n) for n in "uvw"]
+    res = []
+    for shift in ((0, 0), (3, 5)):
+        F = [synth.embed(np.roll(a, shift, axis=(0, 1)), cfg.halo) for a in fs]
+        d = [gc.to_dev(a, L) for a in F]
+        outs = gc.fresh_out(L, 3)
+        L.momentum(*d, *outs)
+        torch.cuda.synchronize()
+        res.append([gc.interior(cfg, o.cpu().numpy()) for o in outs])
+    for a, b in zip(*res):
+        assert np.array_equal(np.roll(a, (3, 5), axis=(0, 1)), b)
+    L.close()
+
+
+def test_user_supplied_tz_arrays_and_stream():
+    cfg = gc.custom_cfg(8, 8, 32, cid=306)
+    g = synth.grid(cfg.nz)
+    P = oracle.Problem(cfg.nx, cfg.ny, cfg.nz, cfg.halo, 50.0, 50.0, g["dz"], g["dzn"], g["rho"], g["rhon"])
+    L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, 50.0, 50.0,
+                        tzc1=P.tzc1, tzc2=P.tzc2, tzd1=P.tzd1, tzd2=P.tzd2)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    d = [gc.to_dev(a, L) for a in (U, V, W)]
+    outs = gc.fresh_out(L, 3)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        L.momentum(*d, *outs, stream=st)
+    st.synchronize()
+    for o, w_, n in zip(outs, P.momentum(U, V, W), ("su", "sv", "sw")):
+        gc.check(cfg, o, w_, n)
+    assert L.launch_count() == 1
+    L.close()
