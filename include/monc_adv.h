@@ -161,11 +161,20 @@ int monc_adv_set_form(monc_adv_t h, int form);
 /* 0 (default): tendencies overwritten.  1: added into the output buffers. */
 int monc_adv_set_accumulate(monc_adv_t h, int on);
 /* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
- * kernels, 2 = x-marching vector kernels (need nz % (16/sizeof(dtype)) == 0). */
+ * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
+ * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need
+ * nz % (16/sizeof(dtype)) == 0 and the flux form. */
 int monc_adv_set_variant(monc_adv_t h, int variant);
-/* Tuning knobs of the x-marching kernels; 0 = library default.
- *   xchunk: planes marched by one thread block;  group: scalars per thread. */
-int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group);
+/* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
+ * that makes sense.
+ *   xchunk:   planes marched by one thread block;
+ *   group:    scalars advected per thread (1..5);
+ *   prefetch: L2 prefetch distance in planes (-1 = no prefetch), variant 2;
+ *   warps:    warps per thread block (1..8), variant 2;
+ *   stages:   depth of the TMA ring (3..8), variant 3;
+ *   tile_y:   columns per thread block, variant 3. */
+int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
+                        int tile_y);
 
 /* Copy the coefficient tables the handle uses to HOST arrays of nz doubles
  * (as stored, i.e. after rounding to fp32 for an F32 handle).  Any pointer

@@ -79,7 +79,7 @@ def load():
                  "monc_adv_set_accumulate", "monc_adv_set_variant"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
-    lib.monc_adv_set_tuning.argtypes = [vp, ci, ci]
+    lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci]
     lib.monc_adv_set_tuning.restype = ci
     lib.monc_adv_get_coefficients.argtypes = [vp] + [dp] * 4
     lib.monc_adv_get_coefficients.restype = ci
@@ -236,11 +236,12 @@ class MoncAdv:
         self._check(self._lib.monc_adv_set_accumulate(self._h, int(bool(on))))
 
     def set_variant(self, variant):
-        variant = {"auto": 0, "generic": 1, "march": 2}.get(variant, variant)
+        variant = {"auto": 0, "generic": 1, "march": 2, "tma": 3}.get(variant, variant)
         self._check(self._lib.monc_adv_set_variant(self._h, int(variant)))
 
-    def set_tuning(self, xchunk=0, group=0):
-        self._check(self._lib.monc_adv_set_tuning(self._h, int(xchunk), int(group)))
+    def set_tuning(self, xchunk=0, group=0, prefetch=0, warps=0, stages=0, tile_y=0):
+        self._check(self._lib.monc_adv_set_tuning(self._h, int(xchunk), int(group), int(prefetch),
+                                                  int(warps), int(stages), int(tile_y)))
 
     def get_coefficients(self):
         import numpy as np

@@ -6,6 +6,7 @@
 // No torch types, no CPU compute fallback: if CUDA fails the call fails.
 #include "monc_adv.h"
 #include "monc_adv_kernels.cuh"
+#include "monc_adv_tma.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -33,7 +34,9 @@ struct monc_adv_s {
   std::vector<double> tz_host[4];                        // as stored on the device
   const void *wind[3] = {nullptr, nullptr, nullptr};
   int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0;
-  int xchunk = 0, group = 0;
+  int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
+  int stages = 0, tile_y = 0;                           // TMA kernels, 0 = default
+  int smem_optin = 0;                                   // max dynamic smem per block
   long launches = 0;
   std::string err;
   // ---- async step state
@@ -79,6 +82,7 @@ KParams<T> make_params(monc_adv_t h, int ia, int ib) {
   p.xc = ib - ia;
   p.accumulate = h->accumulate;
   p.skew = h->form == MONC_ADV_FORM_PW_SKEW;
+  p.prefetch = h->prefetch < 0 ? 0 : (h->prefetch == 0 ? kDefaultPrefetch : h->prefetch);
   p.cx = (T)(1.0 / (4.0 * h->dx));
   p.cy = (T)(1.0 / (4.0 * h->dy));
   p.tzc1 = (const T *)h->d_tz[0]; p.tzc2 = (const T *)h->d_tz[1];
@@ -105,16 +109,76 @@ int pick_xchunk(monc_adv_t h, int nplanes, int blocks_per_plane, int resident_pe
   return std::min(xc, nplanes);
 }
 
+// geometry of the TMA-staged kernels: TY columns per block, ring depth S
+struct TmaPlan {
+  bool ok = false;
+  int ty = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0;
+  size_t smem = 0;
+};
+
+template <typename T>
+TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
+  TmaPlan pl;
+  constexpr int NK = VecOf<T>::NK;
+  if (h->nz % NK != 0) return pl;
+  const int wzc = (h->nz / NK + 31) / 32;
+  if (wzc > kTmaMaxConsumerWarps) return pl;
+  const int tymax = std::min(h->ny, kTmaMaxConsumerWarps / wzc);
+  const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
+  const int ty_hi = h->tile_y > 0 ? std::min(h->tile_y, tymax) : tymax;
+  const int ty_lo = h->tile_y > 0 ? ty_hi : std::max(1, tymax - 3);
+  const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
+  double best = 1e300;
+  for (int ty = ty_hi; ty >= ty_lo; --ty) {
+    const size_t stage = (size_t)fields_per_stage * (ty + 2) * h->nz * sizeof(T);
+    int S = (int)std::min<size_t>(8, budget / (stage + 16));
+    if (h->stages > 0) S = std::min(S, h->stages);
+    if (S < 3) continue;
+    const int tiles = (h->ny + ty - 1) / ty;
+    const int nch_lo = nch_fixed ? nch_fixed : 1;
+    const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 8);
+    for (int nch = nch_lo; nch <= nch_hi; ++nch) {
+      const int xc = (nplanes + nch - 1) / nch;
+      const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
+      const long waves = (blocks + h->sm_count - 1) / h->sm_count;
+      // time ~ waves * (columns per block) * (planes per block + ramp-up planes)
+      const double cost = (double)waves * ty * (xc + 3) * (1.0 + 0.02 * (tymax - ty));
+      if (cost < best) {
+        best = cost;
+        pl.ok = true; pl.ty = ty; pl.stages = S; pl.xc = xc; pl.tiles = tiles;
+        pl.nchunks = (nplanes + xc - 1) / xc;
+        pl.smem = (size_t)S * (stage + 16);
+      }
+    }
+  }
+  return pl;
+}
+
 template <typename T>
 int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
                     int ia, int ib, cudaStream_t st) {
   if (ib <= ia) return MONC_ADV_OK;
   KParams<T> p = make_params<T>(h, ia, ib);
-  if (use_march<T>(h)) {
-    const int bx = (p.units + kWarpsPerBlock - 1) / kWarpsPerBlock;
-    p.xc = pick_xchunk(h, ib - ia, bx, 2, 1);
+  TmaPlan pl;
+  if ((h->variant == 3 || h->variant == 0) && h->form == MONC_ADV_FORM_FLUX)
+    pl = plan_tma<T>(h, ib - ia, 3);
+  if (h->variant == 3 && !pl.ok)
+    return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
+  if (pl.ok) {
+    p.xc = pl.xc;
+    CU(cudaFuncSetAttribute(tma_momentum<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    dim3 grid(pl.tiles, pl.nchunks);
+    tma_momentum<T><<<grid, pl.ty * p.wzc * 32, pl.smem, st>>>(p, pl.ty, pl.stages, u, v, w,
+                                                                     su, sv, sw);
+  } else if (use_march<T>(h)) {
+    const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
+    const int bx = (p.units + wpb - 1) / wpb;
+    p.xc = pick_xchunk(h, ib - ia, bx, 16 / wpb, 1);
     dim3 grid(bx, (ib - ia + p.xc - 1) / p.xc);
-    march_momentum<T><<<grid, kWarpsPerBlock * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+    if (p.wzc > 1)
+      march_momentum<T, true><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+    else
+      march_momentum<T, false><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
   } else {
     const long long n = (long long)(ib - ia) * h->ny * h->nz;
     generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
@@ -126,8 +190,9 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
 
 template <typename T, int G>
 void launch_march_scalars(const KParams<T> &p, const ScalarPtrs<T> &ptrs, int nq, dim3 grid,
-                          int ngroups, const T *u, const T *v, const T *w, cudaStream_t st) {
-  march_scalars<T, G><<<grid, kWarpsPerBlock * 32, 0, st>>>(p, ptrs, nq, ngroups, u, v, w);
+                          int wpb, int ngroups, const T *u, const T *v, const T *w,
+                          cudaStream_t st) {
+  march_scalars<T, G><<<grid, wpb * 32, 0, st>>>(p, ptrs, nq, ngroups, u, v, w);
 }
 
 template <typename T>
@@ -144,15 +209,16 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
     int G = h->group > 0 ? std::min(h->group, 5) : (nq >= 5 ? 5 : nq);
     G = std::min(G, nq);
     const int ngroups = (nq + G - 1) / G;
-    const int bx = (p.units + kWarpsPerBlock - 1) / kWarpsPerBlock;
-    p.xc = pick_xchunk(h, ib - ia, bx, 2, ngroups);
+    const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
+    const int bx = (p.units + wpb - 1) / wpb;
+    p.xc = pick_xchunk(h, ib - ia, bx, 16 / wpb, ngroups);
     dim3 grid(bx * ngroups, (ib - ia + p.xc - 1) / p.xc);
     switch (G) {
-      case 1: launch_march_scalars<T, 1>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
-      case 2: launch_march_scalars<T, 2>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
-      case 3: launch_march_scalars<T, 3>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
-      case 4: launch_march_scalars<T, 4>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
-      default: launch_march_scalars<T, 5>(p, ptrs, nq, grid, ngroups, u, v, w, st); break;
+      case 1: launch_march_scalars<T, 1>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
+      case 2: launch_march_scalars<T, 2>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
+      case 3: launch_march_scalars<T, 3>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
+      case 4: launch_march_scalars<T, 4>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
+      default: launch_march_scalars<T, 5>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
     }
   } else {
     const long long n = (long long)(ib - ia) * h->ny * h->nz;
@@ -348,6 +414,8 @@ int monc_adv_create(monc_adv_t *out, int nx, int ny, int nz, int halo, double dx
   cudaError_t e = cudaGetDevice(&h->device);
   if (e != cudaSuccess) return cfail(e, "cudaGetDevice");
   e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
+  if (e != cudaSuccess) return cfail(e, "cudaDeviceGetAttribute");
+  e = cudaDeviceGetAttribute(&h->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
   if (e != cudaSuccess) return cfail(e, "cudaDeviceGetAttribute");
 
   // ---- coefficient tables (SURVEY.md 8(c).2 "Coefficients"), fp64 on the host
@@ -570,8 +638,8 @@ int monc_adv_set_accumulate(monc_adv_t h, int on) {
 
 int monc_adv_set_variant(monc_adv_t h, int variant) {
   if (!h) return MONC_ADV_EINVAL;
-  if (variant < 0 || variant > 2) return fail(h, MONC_ADV_EINVAL, "set_variant: 0, 1 or 2");
-  if (variant == 2) {
+  if (variant < 0 || variant > 3) return fail(h, MONC_ADV_EINVAL, "set_variant: 0..3");
+  if (variant >= 2) {
     const int nk = h->dtype == MONC_ADV_F64 ? 2 : 4;
     if (h->nz % nk != 0) return fail(h, MONC_ADV_EINVAL, "set_variant: marching kernels need nz % (16/sizeof(dtype)) == 0");
   }
@@ -579,11 +647,18 @@ int monc_adv_set_variant(monc_adv_t h, int variant) {
   return MONC_ADV_OK;
 }
 
-int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group) {
+int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
+                        int tile_y) {
   if (!h) return MONC_ADV_EINVAL;
-  if (xchunk < 0 || group < 0) return fail(h, MONC_ADV_EINVAL, "set_tuning: negative value");
+  if (xchunk < 0 || group < 0 || group > 5 || prefetch < -1 || prefetch > 16 || warps < 0 ||
+      warps > kWarpsPerBlock || stages < 0 || stages > 8 || tile_y < 0)
+    return fail(h, MONC_ADV_EINVAL, "set_tuning: value out of range");
+  h->stages = stages;
+  h->tile_y = tile_y;
   h->xchunk = xchunk;
   h->group = group;
+  h->prefetch = prefetch;
+  h->warps = warps;
   return MONC_ADV_OK;
 }
 

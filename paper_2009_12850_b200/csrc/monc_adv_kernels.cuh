@@ -29,7 +29,8 @@
 namespace monc {
 
 constexpr int kMaxScalars = 64;
-constexpr int kWarpsPerBlock = 8;
+constexpr int kWarpsPerBlock = 8;   // maximum / default
+constexpr int kDefaultPrefetch = 0;  // planes; 0 = off
 
 template <typename T>
 struct KParams {
@@ -42,6 +43,7 @@ struct KParams {
   int units;        // ny * wzc
   int accumulate;   // 0: overwrite, 1: add into outputs
   int skew;         // generic kernels only: PW skew form
+  int prefetch;     // march kernels: L2 prefetch distance in planes (0 = off)
   T cx, cy;         // 1/(4dx), 1/(4dy)
   const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz; tzc2[nz-1] = 0
 };
@@ -107,6 +109,15 @@ __device__ __forceinline__ Vec<T> ld_or_zero(const T *p, bool act) {
 
 constexpr unsigned kFull = 0xffffffffu;
 
+__device__ __forceinline__ void prefetch_l2(const void *p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+// TMA-issued L2 prefetch of a contiguous run (bytes % 16 == 0, 16-B aligned)
+__device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+
 // value one level above each element: r[e] = a[e+1]; the last comes from the
 // next lane's first element, or (warp's last lane) from `edge`.
 template <typename T>
@@ -133,111 +144,154 @@ __device__ __forceinline__ Vec<T> shift_down(const Vec<T> &f, int lane, T edge) 
 }
 
 // ---------------------------------------------------------------------------
-// march_momentum: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks su/sv/sw)
+// One x-step of the fused momentum update for one thread's NK levels.
+// Inputs: centre-plane values C/S/N, east-plane values E, the values one level
+// up (..u), the three fluxes below the thread's first level (b_*: from the
+// previous lane by shuffle, or `edge` values for lane 0) and the west-face
+// fluxes carried from the previous step.  Six distinct face fluxes per point:
+//   fxx (u_i+u_i+1)^2            fyy (v_j+v_j+1)^2           fzz (w_K+w_K+1)^2
+//   fxy (u_j+u_j+1)(v_i+v_i+1)   fxz (u_K+u_K+1)(w_i+w_i+1)  fyz (v_K+v_K+1)(w_j+w_j+1)
+// (FyU == FxV, FzU == FxW, FzV == FyW up to the constant).
+// On return fxx_w/fxy_w/fxz_w hold this step's EAST fluxes (next step's west).
 // ---------------------------------------------------------------------------
 template <typename T>
+__device__ __forceinline__ void momentum_step(
+    const T cx, const T cy, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1,
+    const Vec<T> &d2, const Vec<T> &uC, const Vec<T> &vC, const Vec<T> &vS, const Vec<T> &wC,
+    const Vec<T> &uS, const Vec<T> &uN, const Vec<T> &vN, const Vec<T> &wS, const Vec<T> &wN,
+    const Vec<T> &uE, const Vec<T> &vE, const Vec<T> &vSE, const Vec<T> &wE, const Vec<T> &uCu,
+    const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const T b_xz, const T b_yz,
+    const T b_zz, const int lane, const int k0, const int nz, Vec<T> &fxx_w, Vec<T> &fxy_w,
+    Vec<T> &fxz_w, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> fxx_e, fxy_e, fxz_e, fyz_n, fzz_t, ry, rv, rwy;
+#pragma unroll
+  for (int e = 0; e < NK; ++e) {
+    const T a = uC.v[e] + uE.v[e];
+    fxx_e.v[e] = a * a;                                              // centre i+1
+    fxy_e.v[e] = (uC.v[e] + uN.v[e]) * (vC.v[e] + vE.v[e]);          // corner (i+1/2, j+1/2)
+    const T fxy_se = (uS.v[e] + uC.v[e]) * (vS.v[e] + vSE.v[e]);     // corner (i+1/2, j-1/2)
+    fxz_e.v[e] = (uC.v[e] + uCu.v[e]) * (wC.v[e] + wE.v[e]);         // (i+1/2, z_K)
+    const T bn = vC.v[e] + vN.v[e], bs = vS.v[e] + vC.v[e];
+    fyz_n.v[e] = (vC.v[e] + vCu.v[e]) * (wC.v[e] + wN.v[e]);         // (j+1/2, z_K)
+    const T fyz_s = (vS.v[e] + vSu.v[e]) * (wS.v[e] + wC.v[e]);      // (j-1/2, z_K)
+    const T g = wC.v[e] + wCu.v[e];
+    fzz_t.v[e] = g * g;                                              // at zn_{K+1}
+    ry.v[e] = cy * (fxy_se - fxy_e.v[e]);                            // su: y
+    rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);                            // sw: y
+    rv.v[e] = cx * (fxy_w.v[e] - fxy_e.v[e]) + cy * (bs * bs - bn * bn);  // sv: x + y
+  }
+  const Vec<T> fxz_b = shift_down(fxz_e, lane, b_xz);
+  const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
+  const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
+#pragma unroll
+  for (int e = 0; e < NK; ++e) {
+    const int k = k0 + e;
+    T xu = cx * (fxx_w.v[e] - fxx_e.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * fxz_e.v[e]);
+    T xv = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
+    T xw = cx * (fxz_w.v[e] - fxz_e.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+    if (k == 0) { xu = T(0); xv = T(0); xw = T(0); }
+    if (k == nz - 1) xw = T(0);
+    ou.v[e] = xu; ov.v[e] = xv; ow.v[e] = xw;
+  }
+  fxx_w = fxx_e; fxy_w = fxy_e; fxz_w = fxz_e;
+}
+
+// ---------------------------------------------------------------------------
+// march_momentum: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks su/sv/sw)
+//
+// EDGES = columns span several warps (nz > 32 vectors): lane 31 / lane 0 of a
+// warp read the few scalars of the neighbouring z chunk that a shuffle cannot
+// provide.  Lanes above the column top are clamped onto the last vector: they
+// load valid data, take part in the shuffles and store nothing.
+// ---------------------------------------------------------------------------
+template <typename T, bool EDGES>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict__ v,
                const T *__restrict__ w, T *__restrict__ su, T *__restrict__ sv,
                T *__restrict__ sw) {
   constexpr int NK = VecOf<T>::NK;
   const int lane = threadIdx.x & 31;
-  const int unit = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int unit = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (unit >= p.units) return;  // warp-uniform
   const int jr = unit / p.wzc;
   const int zc = unit - jr * p.wzc;
-  const int k0 = (zc * 32 + lane) * NK;
-  const bool act = k0 < p.nz;
-  const bool top_edge = act && lane == 31 && (k0 + NK < p.nz);
-  const bool bot_edge = act && lane == 0 && zc > 0;
+  const int k0r = (zc * 32 + lane) * NK;
+  const bool act = k0r < p.nz;
+  const int k0 = act ? k0r : p.nz - NK;  // clamp: finite data, never stored
+  const bool top_edge = EDGES && act && lane == 31 && (k0 + NK < p.nz);
+  const bool bot_edge = EDGES && act && lane == 0 && zc > 0;
   const int i0 = p.ia + blockIdx.y * p.xc;
   const int i1 = min(p.ib, i0 + p.xc);
-  const long long nz = p.nz, plane = p.plane;
+  const int nz = p.nz;
+  const long long plane = p.plane;
 
   // per-level coefficients, kept in registers for the whole march
-  Vec<T> c1 = ld_or_zero(p.tzc1 + k0, act), c2 = ld_or_zero(p.tzc2 + k0, act);
-  Vec<T> d1 = ld_or_zero(p.tzd1 + k0, act), d2 = ld_or_zero(p.tzd2 + k0, act);
+  const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+  const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
   const T cx = p.cx, cy = p.cy;
 
-  long long c = ((long long)(i0 - 1) * p.nyh + (jr + p.h)) * nz + k0;  // (i, j, k0)
+  const long long c0 = ((long long)(i0 - 1) * p.nyh + (jr + p.h)) * nz + k0;  // (i0-1, j, k0)
+  const T *pu = u + c0, *pv = v + c0, *pw = w + c0;
+  T *qu = su + c0, *qv = sv + c0, *qw = sw + c0;
   // values of the centre plane that the previous step already loaded
-  Vec<T> uC = ld_or_zero(u + c, act), vC = ld_or_zero(v + c, act);
-  Vec<T> vS = ld_or_zero(v + c - nz, act), wC = ld_or_zero(w + c, act);
+  Vec<T> uC = ld_vec(pu), vC = ld_vec(pv), vS = ld_vec(pv - nz), wC = ld_vec(pw);
   // x-face fluxes on the west side, carried from the previous step
   Vec<T> fxx_w, fxy_w, fxz_w;
 #pragma unroll
   for (int e = 0; e < NK; ++e) fxx_w.v[e] = fxy_w.v[e] = fxz_w.v[e] = T(0);
+  const int pf = p.prefetch;
+  // one lane per warp asks the TMA unit to pull this warp's 32 vectors of
+  // plane i+pf into L2 (DRAM latency then overlaps the steps in between)
+  const bool pf_lane = pf > 0 && lane == 0;
+  const unsigned pf_bytes = (unsigned)(min(32 * NK, nz - k0r) * (int)sizeof(T));
 
 #pragma unroll 1
-  for (int i = i0 - 1; i < i1; ++i, c += plane) {
-    const Vec<T> uS = ld_or_zero(u + c - nz, act), uN = ld_or_zero(u + c + nz, act);
-    const Vec<T> vN = ld_or_zero(v + c + nz, act);
-    const Vec<T> wS = ld_or_zero(w + c - nz, act), wN = ld_or_zero(w + c + nz, act);
-    const Vec<T> uE = ld_or_zero(u + c + plane, act), vE = ld_or_zero(v + c + plane, act);
-    const Vec<T> vSE = ld_or_zero(v + c + plane - nz, act), wE = ld_or_zero(w + c + plane, act);
+  for (int i = i0 - 1; i < i1; ++i) {
+    const Vec<T> uS = ld_vec(pu - nz), uN = ld_vec(pu + nz);
+    const Vec<T> vN = ld_vec(pv + nz);
+    const Vec<T> wS = ld_vec(pw - nz), wN = ld_vec(pw + nz);
+    const Vec<T> uE = ld_vec(pu + plane), vE = ld_vec(pv + plane);
+    const Vec<T> vSE = ld_vec(pv + plane - nz), wE = ld_vec(pw + plane);
+    if (pf_lane && i + pf <= i1) {  // pull plane i+pf of this column towards L2
+      prefetch_l2_bulk(pu + pf * plane, pf_bytes); prefetch_l2_bulk(pv + pf * plane, pf_bytes);
+      prefetch_l2_bulk(pw + pf * plane, pf_bytes);
+    }
     // z-chunk edges: one lane each reads the few scalars a shuffle cannot give
     T e_u = T(0), e_v = T(0), e_w = T(0), e_vs = T(0);
-    if (top_edge) {
-      e_u = __ldg(u + c + NK); e_v = __ldg(v + c + NK);
-      e_w = __ldg(w + c + NK); e_vs = __ldg(v + c - nz + NK);
-    }
     T b_xz = T(0), b_yz = T(0), b_zz = T(0);
-    if (bot_edge) {
-      const T ub = __ldg(u + c - 1), vb = __ldg(v + c - 1), wb = __ldg(w + c - 1);
-      const T web = __ldg(w + c + plane - 1), wnb = __ldg(w + c + nz - 1);
-      b_xz = (ub + uC.v[0]) * (wb + web);
-      b_yz = (vb + vC.v[0]) * (wb + wnb);
-      b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+    if (EDGES) {
+      if (top_edge) {
+        e_u = __ldg(pu + NK); e_v = __ldg(pv + NK);
+        e_w = __ldg(pw + NK); e_vs = __ldg(pv - nz + NK);
+      }
+      if (bot_edge) {
+        const T ub = __ldg(pu - 1), vb = __ldg(pv - 1), wb = __ldg(pw - 1);
+        const T web = __ldg(pw + plane - 1), wnb = __ldg(pw + nz - 1);
+        b_xz = (ub + uC.v[0]) * (wb + web);
+        b_yz = (vb + vC.v[0]) * (wb + wnb);
+        b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+      }
     }
     const Vec<T> uCu = shift_up(uC, lane, e_u), vCu = shift_up(vC, lane, e_v);
     const Vec<T> wCu = shift_up(wC, lane, e_w), vSu = shift_up(vS, lane, e_vs);
 
-    Vec<T> fxx_e, fxy_e, fxz_e, fyz_n, fzz_t, ry, rv, rwy;
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      const T a = uC.v[e] + uE.v[e];
-      fxx_e.v[e] = a * a;                                              // (u_i+u_i+1)^2
-      fxy_e.v[e] = (uC.v[e] + uN.v[e]) * (vC.v[e] + vE.v[e]);          // corner (i+1/2, j+1/2)
-      const T fxy_se = (uS.v[e] + uC.v[e]) * (vS.v[e] + vSE.v[e]);     // corner (i+1/2, j-1/2)
-      fxz_e.v[e] = (uC.v[e] + uCu.v[e]) * (wC.v[e] + wE.v[e]);         // (i+1/2, z_K)
-      const T bn = vC.v[e] + vN.v[e], bs = vS.v[e] + vC.v[e];
-      fyz_n.v[e] = (vC.v[e] + vCu.v[e]) * (wC.v[e] + wN.v[e]);         // (j+1/2, z_K)
-      const T fyz_s = (vS.v[e] + vSu.v[e]) * (wS.v[e] + wC.v[e]);      // (j-1/2, z_K)
-      const T g = wC.v[e] + wCu.v[e];
-      fzz_t.v[e] = g * g;                                              // at zn_{K+1}
-      // horizontal parts
-      ry.v[e] = cy * (fxy_se - fxy_e.v[e]);                            // su: y
-      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);                            // sw: y
-      rv.v[e] = cx * (fxy_w.v[e] - fxy_e.v[e]) + cy * (bs * bs - bn * bn);  // sv: x + y
-    }
-    const Vec<T> fxz_b = shift_down(fxz_e, lane, b_xz);
-    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
-    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
-
+    Vec<T> ou, ov, ow;
+    momentum_step<T>(cx, cy, c1, c2, d1, d2, uC, vC, vS, wC, uS, uN, vN, wS, wN, uE, vE, vSE, wE,
+                     uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, lane, k0, nz, fxx_w, fxy_w, fxz_w, ou,
+                     ov, ow);
     if (i >= i0 && act) {
-      Vec<T> ou, ov, ow;
-#pragma unroll
-      for (int e = 0; e < NK; ++e) {
-        const int k = k0 + e;
-        T xu = cx * (fxx_w.v[e] - fxx_e.v[e]) + ry.v[e] +
-               (c1.v[e] * fxz_b.v[e] - c2.v[e] * fxz_e.v[e]);
-        T xv = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
-        T xw = cx * (fxz_w.v[e] - fxz_e.v[e]) + rwy.v[e] +
-               (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
-        if (k == 0) { xu = T(0); xv = T(0); xw = T(0); }
-        if (k == p.nz - 1) xw = T(0);
-        ou.v[e] = xu; ov.v[e] = xv; ow.v[e] = xw;
-      }
       if (p.accumulate) {
-        const Vec<T> au = ld_vec_rw(su + c), av = ld_vec_rw(sv + c), aw = ld_vec_rw(sw + c);
+        const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
 #pragma unroll
         for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
       }
-      st_vec(su + c, ou); st_vec(sv + c, ov); st_vec(sw + c, ow);
+      st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
     }
     // rotate: east becomes centre
-    fxx_w = fxx_e; fxy_w = fxy_e; fxz_w = fxz_e;
     uC = uE; vC = vE; vS = vSE; wC = wE;
+    pu += plane; pv += plane; pw += plane;
+    qu += plane; qv += plane; qw += plane;
   }
 }
 
@@ -252,21 +306,23 @@ march_scalars(const KParams<T> p, const ScalarPtrs<T> ptrs, const int nq, const 
   constexpr int NK = VecOf<T>::NK;
   const int lane = threadIdx.x & 31;
   const int grp = blockIdx.x % ngroups;  // group index fastest: co-scheduled blocks share the wind in L2
-  const int unit = (blockIdx.x / ngroups) * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int unit = (blockIdx.x / ngroups) * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (unit >= p.units) return;
   const int s0 = grp * G;
   const int cnt = min(G, nq - s0);
   const int jr = unit / p.wzc;
   const int zc = unit - jr * p.wzc;
-  const int k0 = (zc * 32 + lane) * NK;
-  const bool act = k0 < p.nz;
+  const int k0r = (zc * 32 + lane) * NK;
+  const bool act = k0r < p.nz;
+  const int k0 = act ? k0r : p.nz - NK;  // clamp: finite data, never stored
   const bool top_edge = act && lane == 31 && (k0 + NK < p.nz);
   const bool bot_edge = act && lane == 0 && zc > 0;
   const int i0 = p.ia + blockIdx.y * p.xc;
   const int i1 = min(p.ib, i0 + p.xc);
-  const long long nz = p.nz, plane = p.plane;
+  const int nz = p.nz;
+  const long long plane = p.plane;
 
-  Vec<T> c1 = ld_or_zero(p.tzc1 + k0, act), c2 = ld_or_zero(p.tzc2 + k0, act);
+  Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
 #pragma unroll
   for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
   const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
@@ -275,22 +331,34 @@ march_scalars(const KParams<T> p, const ScalarPtrs<T> ptrs, const int nq, const 
   Vec<T> qC[G], fx_w[G];
 #pragma unroll
   for (int s = 0; s < G; ++s) {
-    qC[s] = ld_or_zero(ptrs.q[s0 + (s < cnt ? s : 0)] + c, act);
+    qC[s] = ld_vec(ptrs.q[s0 + (s < cnt ? s : 0)] + c);
 #pragma unroll
     for (int e = 0; e < NK; ++e) fx_w[s].v[e] = T(0);
   }
+  const int pf = p.prefetch;
+  const bool pf_lane = pf > 0 && lane == 0;
+  const unsigned pf_bytes = (unsigned)(min(32 * NK, nz - k0r) * (int)sizeof(T));
 
 #pragma unroll 1
   for (int i = i0 - 1; i < i1; ++i, c += plane) {
-    const Vec<T> uC = ld_or_zero(u + c, act), vC = ld_or_zero(v + c, act);
-    const Vec<T> vS = ld_or_zero(v + c - nz, act), wC = ld_or_zero(w + c, act);
+    const Vec<T> uC = ld_vec(u + c), vC = ld_vec(v + c);
+    const Vec<T> vS = ld_vec(v + c - nz), wC = ld_vec(w + c);
     const T wb = bot_edge ? __ldg(w + c - 1) : T(0);
+    if (pf_lane && i + pf <= i1) {
+      if (grp == 0) {
+        prefetch_l2_bulk(u + c + pf * plane, pf_bytes); prefetch_l2_bulk(v + c + pf * plane, pf_bytes);
+        prefetch_l2_bulk(w + c + pf * plane, pf_bytes);
+      }
+#pragma unroll
+      for (int s = 0; s < G; ++s)
+        if (s < cnt) prefetch_l2_bulk(ptrs.q[s0 + s] + c + (pf + 1) * plane, pf_bytes);
+    }
 #pragma unroll
     for (int s = 0; s < G; ++s) {
       if (s < cnt) {  // block-uniform
         const T *__restrict__ q = ptrs.q[s0 + s];
-        const Vec<T> qE = ld_or_zero(q + c + plane, act);
-        const Vec<T> qS = ld_or_zero(q + c - nz, act), qN = ld_or_zero(q + c + nz, act);
+        const Vec<T> qE = ld_vec(q + c + plane);
+        const Vec<T> qS = ld_vec(q + c - nz), qN = ld_vec(q + c + nz);
         const T e_q = top_edge ? __ldg(q + c + NK) : T(0);
         const T b_z = bot_edge ? wb * (__ldg(q + c - 1) + qC[s].v[0]) : T(0);
         const Vec<T> qCu = shift_up(qC[s], lane, e_q);

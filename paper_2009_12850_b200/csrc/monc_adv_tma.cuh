@@ -1,0 +1,212 @@
+// monc_adv_tma.cuh -- TMA-staged variants of the marching kernels (sm_100a).
+//
+// Same arithmetic as march_momentum / march_scalars (momentum_step is shared),
+// different data movement: a thread block owns TY full columns (+1 halo column
+// on each side) and marches a chunk of x planes.  At fixed x such a tile is ONE
+// contiguous run of (TY+2)*nz elements per field in MONC's z-fastest layout,
+// so a single producer lane streams plane after plane into a shared-memory
+// ring with 1-D bulk TMA copies (cp.async.bulk, SASS UBLKCP) that complete on
+// mbarriers, running several planes ahead of the consumers.  DRAM latency is
+// hidden by the ring depth instead of by registers or occupancy; y neighbours
+// and z-chunk edges are plain shared-memory reads.  There is no dedicated
+// producer warp (a 17th warp would cap the block at 96 registers per thread):
+// lane 0 of the last warp refills, one step late, the slot every warp has
+// released, so the ring runs nstages-2 planes ahead.
+#pragma once
+#include "monc_adv_kernels.cuh"
+
+#include <cstdint>
+
+namespace monc {
+
+constexpr int kTmaMaxConsumerWarps = 16;
+constexpr int kTmaThreads = kTmaMaxConsumerWarps * 32;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(bar), "r"(parity)
+      : "memory");
+}
+// global -> shared bulk copy (bytes % 16 == 0, both addresses 16-B aligned)
+__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void *src, uint32_t bytes,
+                                            uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+      ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+      : "memory");
+}
+
+__device__ __forceinline__ Vec<double> lds_vec(const double *p) {
+  const double2 t = *reinterpret_cast<const double2 *>(p);
+  Vec<double> r;
+  r.v[0] = t.x; r.v[1] = t.y;
+  return r;
+}
+__device__ __forceinline__ Vec<float> lds_vec(const float *p) {
+  const float4 t = *reinterpret_cast<const float4 *>(p);
+  Vec<float> r;
+  r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+  return r;
+}
+// r[e] = a[e+1], last element read from shared memory (level k0 + NK)
+template <typename T>
+__device__ __forceinline__ Vec<T> up_from_smem(const Vec<T> &a, const T *next) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> r;
+#pragma unroll
+  for (int e = 0; e + 1 < NK; ++e) r.v[e] = a.v[e + 1];
+  r.v[NK - 1] = *next;
+  return r;
+}
+
+// dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages mbarriers
+template <typename T>
+__global__ void __launch_bounds__(kTmaThreads, 1)
+tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__restrict__ u,
+             const T *__restrict__ v, const T *__restrict__ w, T *__restrict__ su,
+             T *__restrict__ sv, T *__restrict__ sw) {
+  constexpr int NK = VecOf<T>::NK;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int nz = p.nz;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int fieldsz = (ty + 2) * nz;  // elements of one field in one stage
+  const int stagesz = 3 * fieldsz;
+  T *tiles = reinterpret_cast<T *>(smem_raw);
+  const uint32_t bar0 = smem_u32(smem_raw + (size_t)nstages * stagesz * sizeof(T));
+  // full[s] at bar0 + 8 s, empty[s] at bar0 + 8 (nstages + s)
+  const int jr0 = blockIdx.x * ty;
+  const int ncol = min(ty, p.ny - jr0);
+  const int i0 = p.ia + blockIdx.y * p.xc;
+  const int i1 = min(p.ib, i0 + p.xc);
+  const int nsteps = i1 - i0 + 1;  // consumer steps: planes i0-1 .. i1-1
+  const int ncw = ncol * p.wzc;    // consumer warps that have a column
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < nstages; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      mbar_init(bar0 + 8 * (nstages + s), ncw);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp >= ncw) return;
+  // ---------------- producer role: lane 0 of the last warp ----------------
+  const bool producer = (warp == ncw - 1) && lane == 0;
+  const uint32_t tile_bytes = (uint32_t)((ncol + 2) * nz * (int)sizeof(T));
+  const uint32_t t0 = smem_u32(tiles);
+  long long g_next = ((long long)(i0 - 1) * p.nyh + (jr0 + p.h - 1)) * nz;  // next plane to load
+  int pl_next = 0, s_next = 0;
+  uint32_t par_next = 0;  // parity of the empty-phase the next refill of slot s_next waits for
+  auto issue_plane = [&]() {
+    const uint32_t full = bar0 + 8 * s_next;
+    mbar_expect_tx(full, 3 * tile_bytes);
+    const uint32_t dst = t0 + (uint32_t)(s_next * stagesz * (int)sizeof(T));
+    tma_load_1d(dst, u + g_next, tile_bytes, full);
+    tma_load_1d(dst + (uint32_t)(fieldsz * (int)sizeof(T)), v + g_next, tile_bytes, full);
+    tma_load_1d(dst + (uint32_t)(2 * fieldsz * (int)sizeof(T)), w + g_next, tile_bytes, full);
+    g_next += p.plane;
+    ++pl_next;
+    if (++s_next == nstages) s_next = 0;
+  };
+  if (producer) {
+    const int first = min(nstages, nsteps + 1);  // planes i0-1 .. i1 = nsteps + 1 planes
+    for (int n = 0; n < first; ++n) issue_plane();
+  }
+
+  // ---------------- consumers: warp <-> (column, z chunk) ----------------
+  const int col = warp / p.wzc;
+  const int zc = warp - col * p.wzc;
+  const int k0r = (zc * 32 + lane) * NK;
+  const bool act = k0r < nz;
+  const int k0 = act ? k0r : nz - NK;
+  const bool bot_edge = act && lane == 0 && zc > 0;
+  const int e0 = (col + 1) * nz + k0;  // element index inside a field tile
+  const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+  const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
+  const T cx = p.cx, cy = p.cy;
+  const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+  T *qu = su + c0, *qv = sv + c0, *qw = sw + c0;
+
+  mbar_wait(bar0, 0);  // plane i0-1
+  const T *A = tiles;
+  Vec<T> uC = lds_vec(A + e0), vC = lds_vec(A + fieldsz + e0);
+  Vec<T> vS = lds_vec(A + fieldsz + e0 - nz), wC = lds_vec(A + 2 * fieldsz + e0);
+  Vec<T> fxx_w, fxy_w, fxz_w;
+#pragma unroll
+  for (int e = 0; e < NK; ++e) fxx_w.v[e] = fxy_w.v[e] = fxz_w.v[e] = T(0);
+
+  int sC = 0, sE = 1 % nstages;
+  uint32_t parE = (nstages == 1) ? 1 : 0;
+#pragma unroll 1
+  for (int t = 0; t < nsteps; ++t) {
+    mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
+    const T *B = tiles + sE * stagesz;
+    A = tiles + sC * stagesz;
+    const T *Au = A + e0, *Av = A + fieldsz + e0, *Aw = A + 2 * fieldsz + e0;
+    const Vec<T> uS = lds_vec(Au - nz), uN = lds_vec(Au + nz);
+    const Vec<T> vN = lds_vec(Av + nz);
+    const Vec<T> wS = lds_vec(Aw - nz), wN = lds_vec(Aw + nz);
+    const Vec<T> uE = lds_vec(B + e0), vE = lds_vec(B + fieldsz + e0);
+    const Vec<T> vSE = lds_vec(B + fieldsz + e0 - nz), wE = lds_vec(B + 2 * fieldsz + e0);
+    const Vec<T> uCu = up_from_smem(uC, Au + NK), vCu = up_from_smem(vC, Av + NK);
+    const Vec<T> wCu = up_from_smem(wC, Aw + NK), vSu = up_from_smem(vS, Av - nz + NK);
+    T b_xz = T(0), b_yz = T(0), b_zz = T(0);
+    if (bot_edge) {
+      const T ub = Au[-1], vb = Av[-1], wb = Aw[-1];
+      const T web = B[2 * fieldsz + e0 - 1], wnb = Aw[nz - 1];
+      b_xz = (ub + uC.v[0]) * (wb + web);
+      b_yz = (vb + vC.v[0]) * (wb + wnb);
+      b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+    }
+    Vec<T> ou, ov, ow;
+    momentum_step<T>(cx, cy, c1, c2, d1, d2, uC, vC, vS, wC, uS, uN, vN, wS, wN, uE, vE, vSE, wE,
+                     uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, lane, k0, nz, fxx_w, fxy_w, fxz_w, ou,
+                     ov, ow);
+    // this warp is done with plane i's slot
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
+    if (producer && t >= 1 && pl_next <= nsteps) {
+      // slot of plane i-1: every warp released it during the previous step
+      mbar_wait(bar0 + 8 * (nstages + s_next), par_next);
+      issue_plane();
+      if (s_next == 0) par_next ^= 1;
+    }
+    if (t > 0) {
+      if (act) {
+        if (p.accumulate) {
+          const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
+#pragma unroll
+          for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
+        }
+        st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
+      }
+      qu += p.plane; qv += p.plane; qw += p.plane;
+    }
+    uC = uE; vC = vE; vS = vSE; wC = wE;
+    sC = sE;
+    if (++sE == nstages) { sE = 0; parE ^= 1; }
+  }
+}
+
+}  // namespace monc

@@ -20,10 +20,10 @@ def _need_gpu(gpu_required):
     torch.cuda.synchronize()
 
 
-def run_momentum(cfg, variant="auto", xchunk=0, fields=None, form="flux"):
+def run_momentum(cfg, variant="auto", xchunk=0, fields=None, form="flux", stages=0, tile_y=0):
     P, L = gc.make_pair(cfg)
     L.set_variant(variant)
-    L.set_tuning(xchunk=xchunk)
+    L.set_tuning(xchunk=xchunk, stages=stages, tile_y=tile_y)
     L.set_form(form)
     U, V, W = fields if fields is not None else [synth.field(cfg, n) for n in "uvw"]
     want = P.momentum(U, V, W, skew=(form == "pw_skew"), nthreads=oracle.max_threads())
@@ -63,7 +63,7 @@ def run_scalars(cfg, nq, variant="auto", xchunk=0, group=0, form="flux"):
 # ---------------------------------------------------------------------------
 # BASELINE.json configs 0 and 1: full element-by-element comparison
 # ---------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", ["march", "generic"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
 def test_config0_momentum_fp64(variant):
     run_momentum(synth.CONFIGS[0], variant)
 
@@ -73,9 +73,10 @@ def test_config0_scalars_fp64(variant):
     run_scalars(synth.CONFIGS[0], 4, variant)
 
 
-def test_config1_momentum_fp64_full_size():
-    # the launch configuration bench.py times (variant auto, default tuning)
-    errs = run_momentum(synth.CONFIGS[1])
+@pytest.mark.parametrize("variant", ["auto", "tma", "march"])
+def test_config1_momentum_fp64_full_size(variant):
+    # "auto" is the launch configuration bench.py times (default tuning)
+    errs = run_momentum(synth.CONFIGS[1], variant)
     print("config1 max rel errs", errs)
 
 
@@ -108,6 +109,11 @@ def test_ragged_shapes(shape, dtype):
     cfg = gc.custom_cfg(nx, ny, nz, halo=h, dtype=dtype, cid=200 + nz)
     run_momentum(cfg, "auto", xchunk=0)
     run_momentum(cfg, "auto", xchunk=4)   # several x-chunks: chunk seams
+    vec_ok = nz % (2 if dtype == "f64" else 4) == 0
+    if vec_ok:
+        for variant in ("march", "tma"):
+            run_momentum(cfg, variant, xchunk=0)
+            run_momentum(cfg, variant, xchunk=3, stages=3, tile_y=2)
     run_scalars(cfg, 3, "auto", xchunk=5, group=2)   # ragged group (2 + 1)
 
 
@@ -142,16 +148,16 @@ def test_max_scalars_and_zero():
 # P7 worked example through the library: exact in fp64 AND fp32
 # ---------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("variant", ["march", "generic"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
 def test_P7_exact_through_gpu(dtype, variant):
     from test_oracle_pins import p7_problem, read_golden
     P, (U, V, W, Q) = p7_problem()
     dz = np.array([1, 1, 2, 2, 4, 4], float)
     L = binding.MoncAdv(4, 4, 6, 2, 2.0, 4.0, dz, dz, np.array([1, 1, .5, .5, .25, .25]),
                         np.array([2, 1, 1, .5, .5, .25]), dtype=dtype)
-    if variant == "march" and dtype == "f32":
+    if variant in ("march", "tma") and dtype == "f32":
         with pytest.raises(binding.MoncAdvError):
-            L.set_variant("march")  # nz = 6 is not a multiple of 4
+            L.set_variant(variant)  # nz = 6 is not a multiple of 4
         return
     L.set_variant(variant)
     # coefficient tables as the library stores them
@@ -191,7 +197,7 @@ def test_P7_exact_through_gpu(dtype, variant):
 # ---------------------------------------------------------------------------
 # semantics: accumulate, wind binding, skew form, errors
 # ---------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", ["march", "generic"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
 def test_accumulate_mode(variant):
     cfg = gc.custom_cfg(9, 8, 66, nq=2, cid=302)
     P, L = gc.make_pair(cfg)
