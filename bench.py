@@ -342,7 +342,7 @@ def main():
     ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3"])
     ap.add_argument("--xchunk", type=int, default=0)
     ap.add_argument("--group", type=int, default=0)
-    ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march"])
+    ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march", "tma"])
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--ref-planes", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)

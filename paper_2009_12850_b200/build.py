@@ -15,6 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmonc_adv.so")
 SOURCES = [os.path.join(CSRC, "monc_adv.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "monc_adv_kernels.cuh"),
+                  os.path.join(CSRC, "monc_adv_tma.cuh"),
                   os.path.join(ROOT, "include", "monc_adv.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
