@@ -163,7 +163,8 @@ def run_ours(args):
     g = synth.grid(cfg.nz)
     L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY,
                         g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=cfg.dtype)
-    L.set_tuning(xchunk=args.xchunk, group=args.group)
+    L.set_tuning(xchunk=args.xchunk, group=args.group, stages=args.stages, tile_y=args.tile_y,
+                 warps=args.warps, split=args.split)
     if args.variant:
         L.set_variant(args.variant)
     tdt = L.torch_dtype
@@ -216,6 +217,7 @@ def run_ours(args):
             ev[2 * s + 2].record(st)
     barrier()
     launches = L.launch_count() - n0
+    plan = L.describe_plan()
     total_ms = ev[0].elapsed_time(ev[-1])
     mom_ms = [ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps)]
     sca_ms = [ev[2 * s + 1].elapsed_time(ev[2 * s + 2]) for s in range(args.steps)]
@@ -268,14 +270,16 @@ def run_ours(args):
     sca_b = scalar_bytes_per_pt(cfg.nq, cfg.dtype) * cfg.points if cfg.nq else 0
     mom_avg, sca_avg = float(np.mean(mom_ms)), float(np.mean(sca_ms))
     if sca_b and sca_avg > mom_avg:
-        kern, kb, kms = "march_scalars", sca_b, sca_avg
+        kern, kb, kms = "scalars", sca_b, sca_avg
     else:
-        kern, kb, kms = "march_momentum", mom_b, mom_avg
+        kern, kb, kms = "momentum", mom_b, mom_avg
+    fam = {"": "tma", "auto": "tma", "tma": "tma", "march": "march", "generic": "generic"}[args.variant]
+    tsuf = "double" if cfg.dtype == "f64" else "float"
     achieved = kb / (kms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": f"{fam}_{kern}<{tsuf}>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
-                "best_launch_ms": float(np.min(mom_ms if kern == "march_momentum" else sca_ms)),
+                "best_launch_ms": float(np.min(mom_ms if kern == "momentum" else sca_ms)),
                 "frac_of_nominal_8TBs": achieved / 8000.0}
     kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
     if sca_b:
@@ -293,7 +297,9 @@ def run_ours(args):
                    "halo": cfg.halo, "nq": cfg.nq, "fields_per_step": nf,
                    "l2": f"rotating {nsets} buffer sets ({nsets * 2 * nf * field_bytes / 1e6:.0f} MB) > 126 MB L2",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
-                   "xchunk": args.xchunk, "group": args.group},
+                   "variant": args.variant or "auto", "xchunk": args.xchunk, "group": args.group,
+                   "stages": args.stages, "tile_y": args.tile_y, "warps": args.warps,
+                   "split": args.split, "launch_plan": plan},
         "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
@@ -342,6 +348,10 @@ def main():
     ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3"])
     ap.add_argument("--xchunk", type=int, default=0)
     ap.add_argument("--group", type=int, default=0)
+    ap.add_argument("--stages", type=int, default=0)
+    ap.add_argument("--tile-y", type=int, default=0)
+    ap.add_argument("--warps", type=int, default=0)
+    ap.add_argument("--split", type=int, default=0)
     ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march", "tma"])
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--ref-planes", type=int, default=64)

@@ -168,13 +168,17 @@ int monc_adv_set_variant(monc_adv_t h, int variant);
 /* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
  * that makes sense.
  *   xchunk:   planes marched by one thread block;
- *   group:    scalars advected per thread (1..5);
+ *   group:    scalars that share one staged copy of the wind: per thread block
+ *             (1..10) in variant 3, per thread (1..5) in variant 2;
  *   prefetch: L2 prefetch distance in planes (-1 = no prefetch), variant 2;
- *   warps:    warps per thread block (1..8), variant 2;
- *   stages:   depth of the TMA ring (3..8), variant 3;
- *   tile_y:   columns per thread block, variant 3. */
+ *   warps:    variant 2: warps per thread block (1..8); variant 3 scalars:
+ *             32-vector z chunks per thread block;
+ *   stages:   depth of the TMA ring (2..8), variant 3;
+ *   tile_y:   columns per thread block, variant 3;
+ *   split:    variant 3 scalars: warps that share one column chunk and split
+ *             the block's scalars between them (1..4). */
 int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
-                        int tile_y);
+                        int tile_y, int split);
 
 /* Copy the coefficient tables the handle uses to HOST arrays of nz doubles
  * (as stored, i.e. after rounding to fp32 for an F32 handle).  Any pointer
@@ -183,6 +187,10 @@ int monc_adv_get_coefficients(monc_adv_t h, double *tzc1, double *tzc2, double *
                               double *tzd2);
 /* Kernels launched by this handle since create (the caller's gpu_launches). */
 long monc_adv_launch_count(monc_adv_t h);
+/* Kernel and launch geometry of the last momentum and scalar launches of this
+ * handle (text, for logs and bench records; "" before any launch).  The
+ * pointer stays valid until the next call on the handle. */
+const char *monc_adv_describe_plan(monc_adv_t h);
 /* Text of the last error on this handle ("" if none).  h may be NULL: then the
  * text of the last failed monc_adv_create on this thread. */
 const char *monc_adv_last_error(monc_adv_t h);

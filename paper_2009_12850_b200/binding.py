@@ -31,7 +31,7 @@ SYMBOLS = [
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
-    "monc_adv_last_error", "monc_adv_version",
+    "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version",
 ]
 
 
@@ -79,12 +79,14 @@ def load():
                  "monc_adv_set_accumulate", "monc_adv_set_variant"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
-    lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci]
+    lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
     lib.monc_adv_set_tuning.restype = ci
     lib.monc_adv_get_coefficients.argtypes = [vp] + [dp] * 4
     lib.monc_adv_get_coefficients.restype = ci
     lib.monc_adv_launch_count.argtypes = [vp]
     lib.monc_adv_launch_count.restype = C.c_long
+    lib.monc_adv_describe_plan.argtypes = [vp]
+    lib.monc_adv_describe_plan.restype = C.c_char_p
     lib.monc_adv_last_error.argtypes = [vp]
     lib.monc_adv_last_error.restype = C.c_char_p
     lib.monc_adv_version.argtypes = []
@@ -239,9 +241,9 @@ class MoncAdv:
         variant = {"auto": 0, "generic": 1, "march": 2, "tma": 3}.get(variant, variant)
         self._check(self._lib.monc_adv_set_variant(self._h, int(variant)))
 
-    def set_tuning(self, xchunk=0, group=0, prefetch=0, warps=0, stages=0, tile_y=0):
+    def set_tuning(self, xchunk=0, group=0, prefetch=0, warps=0, stages=0, tile_y=0, split=0):
         self._check(self._lib.monc_adv_set_tuning(self._h, int(xchunk), int(group), int(prefetch),
-                                                  int(warps), int(stages), int(tile_y)))
+                                                  int(warps), int(stages), int(tile_y), int(split)))
 
     def get_coefficients(self):
         import numpy as np
@@ -249,6 +251,9 @@ class MoncAdv:
         self._check(self._lib.monc_adv_get_coefficients(
             self._h, *[o.ctypes.data_as(C.POINTER(C.c_double)) for o in outs]))
         return tuple(outs)
+
+    def describe_plan(self) -> str:
+        return self._lib.monc_adv_describe_plan(self._h).decode()
 
     def launch_count(self) -> int:
         return int(self._lib.monc_adv_launch_count(self._h))

@@ -35,10 +35,11 @@ struct monc_adv_s {
   const void *wind[3] = {nullptr, nullptr, nullptr};
   int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0;
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
-  int stages = 0, tile_y = 0;                           // TMA kernels, 0 = default
+  int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
   long launches = 0;
   std::string err;
+  std::string plan_mom, plan_sca, plan_text;  // geometry of the last launches
   // ---- async step state
   int nchunks = 8, overlap = 1;
   int staged_nq = -1;
@@ -170,6 +171,10 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
     dim3 grid(pl.tiles, pl.nchunks);
     tma_momentum<T><<<grid, pl.ty * p.wzc * 32, pl.smem, st>>>(p, pl.ty, pl.stages, u, v, w,
                                                                      su, sv, sw);
+    char b[160];
+    snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d threads=%d smem=%zu", pl.ty,
+             pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.ty * p.wzc * 32, pl.smem);
+    h->plan_mom = b;
   } else if (use_march<T>(h)) {
     const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
     const int bx = (p.units + wpb - 1) / wpb;
@@ -179,12 +184,187 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
       march_momentum<T, true><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
     else
       march_momentum<T, false><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+    h->plan_mom = "march_momentum xc=" + std::to_string(p.xc);
   } else {
+    h->plan_mom = "generic_momentum";
     const long long n = (long long)(ib - ia) * h->ny * h->nz;
     generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
   }
   CU(cudaGetLastError());
   h->launches++;
+  return MONC_ADV_OK;
+}
+
+// ---- tensor-map encoder, fetched from the driver at first use (no -lcuda link)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn tensor_map_encoder() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void *sym = nullptr;
+    cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      return nullptr;
+    }
+    return reinterpret_cast<EncodeTiledFn>(sym);
+  }();
+  return fn;
+}
+
+// descriptor of one field F[NXH][NYH][nz] with a (z, y, x) box of box_z x box_y x 1
+template <typename T>
+bool encode_field_map(monc_adv_t h, CUtensorMap *m, const void *base, int box_z, int box_y) {
+  EncodeTiledFn enc = tensor_map_encoder();
+  if (!enc) return false;
+  const cuuint64_t gdim[3] = {(cuuint64_t)h->nz, (cuuint64_t)h->nyh, (cuuint64_t)h->nxh};
+  const cuuint64_t gstr[2] = {(cuuint64_t)h->nz * sizeof(T), (cuuint64_t)h->nyh * h->nz * sizeof(T)};
+  const cuuint32_t box[3] = {(cuuint32_t)box_z, (cuuint32_t)box_y, 1u};
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  const CUtensorMapDataType dt =
+      sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  return enc(m, dt, 3, const_cast<void *>(base), gdim, gstr, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// geometry of tma_scalars: ty columns x zw z-chunks (32 vectors each) x ss
+// scalar splits = consumer warps per block; gb scalars per block (gw per
+// warp); ring depth S.  A stage holds 3 + gb field tiles of (ty+2) rows of
+// ZB + 2*NK elements (each tile rounded up to 128 B).
+struct TmaScalarPlan {
+  bool ok = false;
+  int ty = 0, zw = 0, ss = 0, gb = 0, gw = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0, fieldsz = 0;
+  size_t smem = 0;
+};
+
+template <typename T>
+TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
+  TmaScalarPlan pl;
+  constexpr int NK = VecOf<T>::NK;
+  if (h->nz % NK != 0 || !tensor_map_encoder()) return pl;
+  const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
+  const int wzc = (h->nz / NK + 31) / 32;  // warps a whole column needs
+  const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
+  const int zwmax = std::min({wzc, kScalarConsumerWarps, (256 - 2 * NK) / (32 * NK)});  // box dim <= 256
+  double best = 1e300;
+  // Cost model, calibrated on B200:
+  // a block step (one plane) takes max(DRAM time of its bytes at this SM's share
+  // of HBM bandwidth, the serial time of one warp's gw scalars), stretched when
+  // the ring is shallow, plus a fixed synchronisation cost; a launch takes
+  // waves * (planes per block + 2) steps.
+  const double sm_gbs = 6200.0 / h->sm_count;
+  for (int gb = std::min(n, 10); gb >= 1; --gb) {
+    if (h->group > 0 && gb != std::min(h->group, std::min(n, 10))) continue;
+    if (h->group == 0 && gb != std::min(n, 5) && gb != std::min(n, 10)) continue;
+    const int ngroups = (n + gb - 1) / gb;
+    for (int ss = 1; ss <= std::min(gb, 4); ++ss) {
+      if (h->split > 0 && ss != std::min(h->split, std::min(gb, 4))) continue;
+      const int gw = (gb + ss - 1) / ss;
+      if (gw > 5) continue;
+      for (int zw = 1; zw <= zwmax; ++zw) {
+        if (h->warps > 0 && zw != std::min(h->warps, zwmax)) continue;
+        const int ZB = zw * 32 * NK, RS = ZB + 2 * NK;
+        const int nzt = (h->nz + ZB - 1) / ZB;
+        const int tymax = std::min(h->ny, kScalarConsumerWarps / (zw * ss));
+        if (tymax < 1) continue;
+        for (int ty = tymax; ty >= 1; --ty) {
+          if (h->tile_y > 0 && ty != std::min(h->tile_y, tymax)) continue;
+          const size_t field = ((size_t)(ty + 2) * RS * sizeof(T) + 127) / 128 * 128;
+          const size_t stage = (size_t)(3 + gb) * field;
+          int S = (int)std::min<size_t>(8, budget / (stage + 16));
+          if (h->stages > 0) S = std::min(S, h->stages);
+          if (S < 2) continue;
+          const int tiles = ((h->ny + ty - 1) / ty) * nzt * ngroups;
+          const double dram_b = ((3.0 / ngroups + gb) + gb) * ty * ZB * sizeof(T);  // wind shared via L2
+          const double t_mem = dram_b / (sm_gbs * 1e3);                            // us
+          const double t_warp = 0.15 + 0.30 * gw;                                    // us
+          const double shallow = S >= 5 ? 1.0 : (S == 4 ? 1.10 : (S == 3 ? 1.15 : 1.5));
+          const double t_step = std::max(t_mem, t_warp) * shallow + 0.05;
+          const int nch_lo = nch_fixed ? nch_fixed : 1;
+          const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 8);
+          for (int nch = nch_lo; nch <= nch_hi; ++nch) {
+            const int xc = (nplanes + nch - 1) / nch;
+            const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
+            const long waves = (blocks + h->sm_count - 1) / h->sm_count;
+            const double cost = (double)waves * (xc + 2) * t_step;
+            if (cost < best) {
+              best = cost;
+              pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
+              pl.xc = xc; pl.tiles = tiles;
+              pl.nchunks = (nplanes + xc - 1) / xc;
+              pl.fieldsz = (int)(field / sizeof(T));
+              pl.smem = (size_t)S * (stage + 16);
+            }
+          }
+        }
+      }
+    }
+  }
+  return pl;
+}
+
+template <typename T, int GW>
+int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
+                       const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+  CU(cudaFuncSetAttribute(tma_scalars<T, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+  dim3 grid(pl.tiles, pl.nchunks);
+  const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
+  tma_scalars<T, GW><<<grid, threads, pl.smem, st>>>(p, maps, outs, nq, (nq + pl.gb - 1) / pl.gb,
+                                                     pl.gb, pl.ty, pl.zw, pl.ss, pl.stages,
+                                                     pl.fieldsz);
+  return MONC_ADV_OK;
+}
+
+// One launch of tma_scalars per kMaxScalarsPerLaunch scalars.  *done = false
+// with MONC_ADV_OK means "does not fit, nothing launched": the caller falls back.
+template <typename T>
+int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T *w,
+                    const void *const *q, void *const *sq, int nq, int ia, int ib,
+                    cudaStream_t st, bool *done) {
+  *done = false;
+  constexpr int NK = VecOf<T>::NK;
+  for (int base = 0; base < nq; base += kMaxScalarsPerLaunch) {
+    const int n = std::min(kMaxScalarsPerLaunch, nq - base);
+    const TmaScalarPlan pl = plan_tma_scalars<T>(h, ib - ia, n);
+    if (!pl.ok) {
+      if (base == 0) return MONC_ADV_OK;
+      return fail(h, MONC_ADV_ECUDA, "scalars: TMA plan failed after a partial launch");
+    }
+    const int RS = pl.zw * 32 * NK + 2 * NK;
+    TensorMaps maps;
+    SqPtrs<T> outs;
+    bool ok = encode_field_map<T>(h, &maps.m[0], u, RS, pl.ty + 2) &&
+              encode_field_map<T>(h, &maps.m[1], v, RS, pl.ty + 2) &&
+              encode_field_map<T>(h, &maps.m[2], w, RS, pl.ty + 2);
+    for (int s = 0; s < kMaxScalarsPerLaunch; ++s) {
+      const int src = base + (s < n ? s : 0);
+      ok = ok && encode_field_map<T>(h, &maps.m[3 + s], q[src], RS, pl.ty + 2);
+      outs.sq[s] = (T *)sq[src];
+    }
+    if (!ok) return fail(h, MONC_ADV_ECUDA, "scalars: cuTensorMapEncodeTiled failed");
+    p.xc = pl.xc;
+    int rc = MONC_ADV_OK;
+    switch (pl.gw) {
+      case 1: rc = launch_tma_scalars<T, 1>(h, p, maps, outs, n, pl, st); break;
+      case 2: rc = launch_tma_scalars<T, 2>(h, p, maps, outs, n, pl, st); break;
+      case 3: rc = launch_tma_scalars<T, 3>(h, p, maps, outs, n, pl, st); break;
+      case 4: rc = launch_tma_scalars<T, 4>(h, p, maps, outs, n, pl, st); break;
+      default: rc = launch_tma_scalars<T, 5>(h, p, maps, outs, n, pl, st); break;
+    }
+    if (rc != MONC_ADV_OK) return rc;
+    CU(cudaGetLastError());
+    h->launches++;
+    char b[200];
+    snprintf(b, sizeof b, "tma_scalars group=%d per_warp=%d split=%d ty=%d zw=%d stages=%d xc=%d grid=%dx%d "
+             "threads=%d smem=%zu", pl.gb, pl.gw, pl.ss, pl.ty, pl.zw, pl.stages, pl.xc, pl.tiles,
+             pl.nchunks, (pl.ty * pl.zw * pl.ss + 1) * 32, pl.smem);
+    h->plan_sca = b;
+  }
+  *done = true;
   return MONC_ADV_OK;
 }
 
@@ -205,6 +385,13 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
     ptrs.q[n] = (const T *)q[n < nq ? n : 0];
     ptrs.sq[n] = (T *)sq[n < nq ? n : 0];
   }
+  if ((h->variant == 3 || h->variant == 0) && h->form == MONC_ADV_FORM_FLUX) {
+    bool done = false;
+    const int rc = run_tma_scalars<T>(h, p, u, v, w, q, sq, nq, ia, ib, st, &done);
+    if (rc != MONC_ADV_OK || done) return rc;
+  }
+  if (h->variant == 3)
+    return fail(h, MONC_ADV_EINVAL, "scalars: TMA variant does not fit this nz / form");
   if (use_march<T>(h)) {
     int G = h->group > 0 ? std::min(h->group, 5) : (nq >= 5 ? 5 : nq);
     G = std::min(G, nq);
@@ -220,7 +407,9 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
       case 4: launch_march_scalars<T, 4>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
       default: launch_march_scalars<T, 5>(p, ptrs, nq, grid, wpb, ngroups, u, v, w, st); break;
     }
+    h->plan_sca = "march_scalars group=" + std::to_string(G) + " xc=" + std::to_string(p.xc);
   } else {
+    h->plan_sca = "generic_scalars";
     const long long n = (long long)(ib - ia) * h->ny * h->nz;
     dim3 grid((unsigned)((n + 255) / 256), nq);
     generic_scalars<T><<<grid, 256, 0, st>>>(p, ptrs, u, v, w);
@@ -648,11 +837,12 @@ int monc_adv_set_variant(monc_adv_t h, int variant) {
 }
 
 int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
-                        int tile_y) {
+                        int tile_y, int split) {
   if (!h) return MONC_ADV_EINVAL;
-  if (xchunk < 0 || group < 0 || group > 5 || prefetch < -1 || prefetch > 16 || warps < 0 ||
-      warps > kWarpsPerBlock || stages < 0 || stages > 8 || tile_y < 0)
+  if (xchunk < 0 || group < 0 || group > 10 || prefetch < -1 || prefetch > 16 || warps < 0 ||
+      warps > kWarpsPerBlock || stages < 0 || stages > 8 || tile_y < 0 || split < 0 || split > 4)
     return fail(h, MONC_ADV_EINVAL, "set_tuning: value out of range");
+  h->split = split;
   h->stages = stages;
   h->tile_y = tile_y;
   h->xchunk = xchunk;
@@ -672,6 +862,12 @@ int monc_adv_get_coefficients(monc_adv_t h, double *tzc1, double *tzc2, double *
 }
 
 long monc_adv_launch_count(monc_adv_t h) { return h ? h->launches : 0; }
+
+const char *monc_adv_describe_plan(monc_adv_t h) {
+  if (!h) return "";
+  h->plan_text = h->plan_mom + (h->plan_mom.empty() || h->plan_sca.empty() ? "" : "; ") + h->plan_sca;
+  return h->plan_text.c_str();
+}
 
 const char *monc_adv_last_error(monc_adv_t h) {
   return h ? h->err.c_str() : g_create_error.c_str();

@@ -15,6 +15,8 @@
 #pragma once
 #include "monc_adv_kernels.cuh"
 
+#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched at run time)
+
 #include <cstdint>
 
 namespace monc {
@@ -206,6 +208,223 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     uC = uE; vC = vE; vS = vSE; wC = wE;
     sC = sE;
     if (++sE == nstages) { sE = 0; parE ^= 1; }
+  }
+}
+
+}  // namespace monc
+
+namespace monc {
+
+// ---------------------------------------------------------------------------
+// Tensor-map TMA (cp.async.bulk.tensor, SASS UTMALDG): one instruction moves a
+// (z, y) box of one x plane of one field, strided rows and all, and fills
+// out-of-range elements (levels below 0 / above nz-1, rows past the array)
+// with zeros.  Descriptors are encoded on the host per call (the field
+// pointers are call arguments) and passed as __grid_constant__ parameters.
+// ---------------------------------------------------------------------------
+constexpr int kMaxScalarsPerLaunch = 20;  // 23 descriptors of 128 B stay below the 4 KB parameter limit
+
+struct alignas(64) TensorMaps {
+  CUtensorMap m[3 + kMaxScalarsPerLaunch];  // u, v, w, then the scalars of this launch
+};
+template <typename T>
+struct SqPtrs {
+  T *sq[kMaxScalarsPerLaunch];
+};
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, int c0, int c1,
+                                            int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+      " [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+// ---------------------------------------------------------------------------
+// tma_scalars<GW>: batched scalar tendencies (SURVEY.md 8(a) row a2, 8(c).2
+// block sq; PAPER.md:83 wind shared by kernels).
+//
+// A block owns a (y, z) tile of `ty` columns x ZB = zw*32*NK levels, advects
+// gb = GW*ss scalars of one group and marches a chunk of x planes.  A stage of
+// the ring holds, for u, v, w and the gb scalars, the box rows [jr0-1, jr0+ty]
+// x levels [kb0-NK, kb0+ZB+NK) of ONE plane: one tensor-map TMA copy per field,
+// issued by a dedicated producer warp (lanes 0..2+gb), completing on the
+// stage's `full` mbarrier.  Elements outside the array are zero-filled by the
+// TMA unit: they are read (the top level's upper neighbour) but multiplied by
+// a zero coefficient.
+//
+// Consumer warp <-> (column, 32-vector z chunk, scalar split): `ss` warps share
+// one column chunk and take GW scalars each, so the warp count (latency hiding)
+// does not shrink when the tile is made small enough for a deep ring.
+//
+// Every plane is touched in exactly ONE consumer step (so S-1 of the S stages
+// can be in flight): when plane i lands a thread forms, per scalar, the y and z
+// flux differences of plane i (kept in registers as P) and the x flux through
+// the face between planes i-1 and i from the carried q(i-1), u(i-1); with the
+// carried P(i-1) and west flux that completes sq(i-1), which is stored.
+//
+// dynamic shared memory: nstages * (3+gb) field tiles of fieldsz elements
+// ((ty+2)*(ZB+2NK) rounded up to 128 B), then 2*nstages mbarriers.
+// ---------------------------------------------------------------------------
+// 15 consumer warps + the producer warp = 512 threads: 128 registers per thread
+constexpr int kScalarConsumerWarps = 15;
+constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
+
+template <typename T, int GW>
+__global__ void __launch_bounds__(kScalarThreads, 1)
+tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
+            const int nq, const int ngroups, const int gb, const int ty, const int zw,
+            const int ss, const int nstages, const int fieldsz) {
+  constexpr int NK = VecOf<T>::NK;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int nz = p.nz;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ZB = zw * 32 * NK;   // levels per block tile
+  const int RS = ZB + 2 * NK;    // row stride: one 16-byte vector of z halo on each side
+  const int rows = ty + 2;
+  const int stagesz = (3 + gb) * fieldsz;
+  T *tiles = reinterpret_cast<T *>(smem_raw);
+  const uint32_t bar0 = smem_u32(smem_raw + (size_t)nstages * stagesz * sizeof(T));
+  // full[s] at bar0 + 8 s, empty[s] at bar0 + 8 (nstages + s)
+
+  // block -> (scalar group, z tile, y tile); group fastest so that the blocks
+  // sharing a wind tile run together and the later reads hit L2
+  const int grp = blockIdx.x % ngroups;
+  const int tile = blockIdx.x / ngroups;
+  const int nzt = (nz + ZB - 1) / ZB;
+  const int zt = tile % nzt, yt = tile / nzt;
+  const int s0 = grp * gb;
+  const int cnt = min(gb, nq - s0);  // scalars of this block
+  const int jr0 = yt * ty;
+  const int ncol = min(ty, p.ny - jr0);
+  const int kb0 = zt * ZB;
+  const int zlive = min(zw, (nz - kb0 + 32 * NK - 1) / (32 * NK));  // z chunks with a level < nz
+  const int slive = (cnt + GW - 1) / GW;                             // splits with a scalar
+  const int ncw = ncol * zlive * slive;                              // live consumer warps
+  const int i0 = p.ia + blockIdx.y * p.xc;
+  const int i1 = min(p.ib, i0 + p.xc);
+  const int nplanes = i1 - i0 + 2;  // planes i0-1 .. i1
+  const int nwarps_c = ty * zw * ss;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < nstages; ++s) {
+      mbar_init(bar0 + 8 * s, 1);
+      mbar_init(bar0 + 8 * (nstages + s), ncw);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == nwarps_c) {
+    // ---------------- producer warp: one lane per field ----------------
+    const int nfld = 3 + cnt;
+    const uint32_t box_bytes = (uint32_t)(rows * RS * (int)sizeof(T));
+    const CUtensorMap *mymap = &maps.m[lane < 3 ? lane : 3 + s0 + min(lane - 3, cnt - 1)];
+    if (lane < nfld) prefetch_tensormap(mymap);
+    const uint32_t t0 = smem_u32(tiles);
+    int s = 0;
+    uint32_t par = 1;  // a fresh mbarrier passes a wait on parity 1: the first lap does not block
+#pragma unroll 1
+    for (int n = 0; n < nplanes; ++n) {
+      mbar_wait(bar0 + 8 * (nstages + s), par);  // every consumer warp released the slot
+      const uint32_t full = bar0 + 8 * s;
+      if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
+      __syncwarp();
+      if (lane < nfld)
+        tma_load_3d(t0 + (uint32_t)((s * stagesz + lane * fieldsz) * (int)sizeof(T)), mymap,
+                    kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+      if (++s == nstages) { s = 0; par ^= 1; }
+    }
+    return;
+  }
+
+  // ---------------- consumers ----------------
+  const int col = warp / (zw * ss);
+  const int rem = warp - col * (zw * ss);
+  const int zc = rem / ss;
+  const int sp = rem - zc * ss;
+  if (col >= ncol || zc >= zlive || sp >= slive) return;
+  const int sb = sp * GW;              // first scalar (within the block's group) of this warp
+  const int mycnt = min(GW, cnt - sb);
+  const int k0r = kb0 + (zc * 32 + lane) * NK;
+  const bool act = k0r < nz;
+  const int k0 = act ? k0r : nz - NK;  // clamp: finite data, never stored
+  const bool bot_edge = act && lane == 0 && k0 > 0;
+  const int e0 = (col + 1) * RS + (k0 - (kb0 - NK));  // element index inside a field tile
+  Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+#pragma unroll
+  for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
+  const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
+  long long c = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+
+  Vec<T> uP, qP[GW], fxP[GW], P[GW];  // carried from the previous plane
+#pragma unroll
+  for (int e = 0; e < NK; ++e) uP.v[e] = T(0);
+#pragma unroll
+  for (int s = 0; s < GW; ++s) {
+#pragma unroll
+    for (int e = 0; e < NK; ++e) qP[s].v[e] = fxP[s].v[e] = P[s].v[e] = T(0);
+  }
+
+  int st = 0;
+  uint32_t par = 0;
+#pragma unroll 1
+  for (int t = 0; t < nplanes; ++t) {
+    mbar_wait(bar0 + 8 * st, par);  // plane i0-1+t has landed
+    const T *A = tiles + st * stagesz + e0;
+    const Vec<T> uC = lds_vec(A), vC = lds_vec(A + fieldsz);
+    const Vec<T> vS = lds_vec(A + fieldsz - RS), wC = lds_vec(A + 2 * fieldsz);
+    const T wb = bot_edge ? A[2 * fieldsz - 1] : T(0);
+    const bool store = act && t >= 2;
+#pragma unroll
+    for (int s = 0; s < GW; ++s) {
+      if (s < mycnt) {  // warp-uniform
+        const T *Aq = A + (3 + sb + s) * fieldsz;
+        const Vec<T> q = lds_vec(Aq);
+        const Vec<T> qS = lds_vec(Aq - RS), qN = lds_vec(Aq + RS);
+        const Vec<T> qU = up_from_smem(q, Aq + NK);
+        const T b_z = bot_edge ? wb * (Aq[-1] + q.v[0]) : T(0);
+        Vec<T> fx, fz_t, hy;
+#pragma unroll
+        for (int e = 0; e < NK; ++e) {
+          fx.v[e] = uP.v[e] * (qP[s].v[e] + q.v[e]);  // face between planes i-1 and i
+          hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + q.v[e]) - vC.v[e] * (q.v[e] + qN.v[e]));
+          fz_t.v[e] = wC.v[e] * (q.v[e] + qU.v[e]);
+        }
+        const Vec<T> fz_b = shift_down(fz_t, lane, b_z);
+        if (store) {  // sq of plane i-1 is complete
+          Vec<T> o;
+#pragma unroll
+          for (int e = 0; e < NK; ++e) {
+            T x = P[s].v[e] + cx2 * (fxP[s].v[e] - fx.v[e]);
+            if (k0 + e == 0) x = T(0);
+            o.v[e] = x;
+          }
+          T *sq = outs.sq[s0 + sb + s] + c;
+          if (p.accumulate) {
+            const Vec<T> a = ld_vec_rw(sq);
+#pragma unroll
+            for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
+          }
+          st_vec(sq, o);
+        }
+#pragma unroll
+        for (int e = 0; e < NK; ++e)
+          P[s].v[e] = hy.v[e] + (c1.v[e] * fz_b.v[e] - c2.v[e] * fz_t.v[e]);
+        qP[s] = q;
+        fxP[s] = fx;
+      }
+    }
+    uP = uC;
+    // this warp is done with the slot
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
+    if (t >= 2) c += p.plane;
+    if (++st == nstages) { st = 0; par ^= 1; }
   }
 }
 

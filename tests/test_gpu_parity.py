@@ -38,11 +38,12 @@ def run_momentum(cfg, variant="auto", xchunk=0, fields=None, form="flux", stages
     return errs
 
 
-def run_scalars(cfg, nq, variant="auto", xchunk=0, group=0, form="flux"):
+def run_scalars(cfg, nq, variant="auto", xchunk=0, group=0, form="flux", stages=0, tile_y=0, warps=0,
+                split=0):
     cfgq = dataclasses.replace(cfg, nq=nq)
     P, L = gc.make_pair(cfgq)
     L.set_variant(variant)
-    L.set_tuning(xchunk=xchunk, group=group)
+    L.set_tuning(xchunk=xchunk, group=group, stages=stages, tile_y=tile_y, warps=warps, split=split)
     L.set_form(form)
     U, V, W = [synth.field(cfgq, n) for n in "uvw"]
     names = synth.field_names(cfgq)
@@ -68,7 +69,7 @@ def test_config0_momentum_fp64(variant):
     run_momentum(synth.CONFIGS[0], variant)
 
 
-@pytest.mark.parametrize("variant", ["march", "generic"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
 def test_config0_scalars_fp64(variant):
     run_scalars(synth.CONFIGS[0], 4, variant)
 
@@ -115,12 +116,29 @@ def test_ragged_shapes(shape, dtype):
             run_momentum(cfg, variant, xchunk=0)
             run_momentum(cfg, variant, xchunk=3, stages=3, tile_y=2)
     run_scalars(cfg, 3, "auto", xchunk=5, group=2)   # ragged group (2 + 1)
+    if vec_ok:
+        run_scalars(cfg, 3, "march", xchunk=5, group=2)
+        # TMA ring: z split over 1 or 2 warps per column per block (ragged last z
+        # tile), short ring, ragged y tiles, several x chunks
+        run_scalars(cfg, 3, "tma", xchunk=0, group=3)
+        run_scalars(cfg, 3, "tma", xchunk=3, group=2, stages=2, tile_y=2, warps=1, split=1)
+        run_scalars(cfg, 4, "tma", xchunk=4, group=3, stages=4, tile_y=3, warps=2, split=2)
+        run_scalars(cfg, 7, "tma", xchunk=2, group=7, stages=3, tile_y=2, warps=1, split=3)
 
 
+@pytest.mark.parametrize("variant", ["tma", "march"])
 @pytest.mark.parametrize("group", [1, 2, 3, 4, 5])
-def test_scalar_group_sizes(group):
+def test_scalar_group_sizes(group, variant):
     cfg = gc.custom_cfg(12, 9, 70, nq=7, cid=300)
-    run_scalars(cfg, 7, "march", xchunk=5, group=group)
+    run_scalars(cfg, 7, variant, xchunk=5, group=group)
+
+
+@pytest.mark.parametrize("group,split", [(10, 2), (10, 3), (10, 4), (9, 2), (6, 3), (5, 1), (4, 4), (7, 2)])
+def test_scalar_block_groups_and_splits(group, split):
+    """tma_scalars: `group` scalars per block shared between `split` warps per
+    column chunk, ragged last group and ragged last split."""
+    cfg = gc.custom_cfg(9, 10, 72, nq=11, cid=302)
+    run_scalars(cfg, 11, "tma", xchunk=4, group=group, split=split)
 
 
 def test_max_scalars_and_zero():
