@@ -50,19 +50,61 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    """SM clock and throttle reasons DURING the timed region: NVML polled from a
+    thread every few ms (the timed region of config1 is milliseconds long, too
+    short for `nvidia-smi -lms`); falls back to the recipe's nvidia-smi line."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
-        self.rows, self.proc, self.index = [], None, index
+    def __init__(self, index=0, period_s=0.004):
+        self.rows, self.proc, self.index, self.period = [], None, index, period_s
+        self.sm, self.reasons, self.mx, self.power = [], set(), None, []
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        try:
+            return int(vis.split(",")[self.index]) if vis else self.index
+        except Exception:
+            return self.index
 
     def start(self):
         try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self._physical_index())
+            self.mx = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            bits = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown,
+                    "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                    "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown,
+                    "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+
+            def poll():
+                while not self._stop.is_set():
+                    try:
+                        self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                        r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                        for name, b in bits.items():
+                            if r & b:
+                                self.reasons.add(name)
+                        self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    except Exception:
+                        pass
+                    self._stop.wait(self.period)
+
+            self._nvml = nv
+            self._thr = threading.Thread(target=poll, daemon=True)
+            self._thr.start()
+            return
+        except Exception:
+            self._nvml = None
+        try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                 "-i", str(self._physical_index()), "-lms", "100"], stdout=subprocess.PIPE, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
@@ -72,6 +114,13 @@ class ClockSampler:
             self.rows.append([x.strip() for x in line.split(",")])
 
     def stop(self):
+        if self._nvml is not None:
+            self._stop.set()
+            self._thr.join(timeout=1.0)
+            return {"sm_mhz": float(np.median(self.sm)) if self.sm else None,
+                    "sm_min_mhz": float(np.min(self.sm)) if self.sm else None, "sm_max_mhz": self.mx,
+                    "power_w_max": float(np.max(self.power)) if self.power else None,
+                    "samples": len(self.sm), "reasons": sorted(self.reasons), "source": "nvml"}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
@@ -87,12 +136,22 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "reasons": sorted(reasons), "source": "nvidia-smi"}
 
 
 def workload_cfg(name):
     from paper_2009_12850_b200 import synth
-    return synth.CONFIGS[{"config1": 1, "config2": 2, "config3": 3}[name]]
+    return synth.CONFIGS[{"config1": 1, "config2": 2, "config3": 3, "config4": 4}[name]]
+
+
+# ncu `dram__bytes_read.sum + dram__bytes_write.sum` per launch of the dominant
+# kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
+# by (workload, kernel family); valid for the library's default launch plan only.
+NCU_TRAFFIC = {
+    ("config1", "tma_momentum"): (359.5e6, "profiles/r01_config1_tma_momentum_f64.md"),
+    ("config2", "tma_scalars"): (13397.5e6, "profiles/r01_config2_tma_scalars_f64.md"),
+    ("config3", "tma_scalars"): (6202.3e6, "profiles/r01_config3_tma_f32.md"),
+}
 
 
 # ---------------------------------------------------------------------------
@@ -171,9 +230,20 @@ def run_ours(args):
     # weak scaling: every rank advects its own subdomain of the config's size
     # ("replicas only" until the halo-exchange row of SURVEY.md 8(f) is built);
     # rank-keyed seed so ranks do not share data
-    rcfg = cfg if rank == 0 else __import__("dataclasses").replace(cfg, seed_cid=1000 + rank)
+    import dataclasses
+    from paper_2009_12850_b200 import dist as pdist
     names = ["u", "v", "w"] + synth.field_names(cfg)
-    H = [synth.field(rcfg, n) for n in names]
+    if args.halo_exchange:
+        # one periodic global domain of world * nx planes, x-slab per rank; the halo
+        # swap runs inside every timed step
+        gcfg = dataclasses.replace(cfg, nx=world * cfg.nx)
+        H = []
+        for n in names:
+            f = pdist.local_from_global(synth.interior_field(gcfg, n), cfg.halo, world, rank)
+            H.append(pdist.fill_halo_y_periodic(f, cfg.halo).numpy())
+    else:
+        rcfg = cfg if rank == 0 else dataclasses.replace(cfg, seed_cid=1000 + rank)
+        H = [synth.field(rcfg, n) for n in names]
     nf = len(names)
     field_bytes = cfg.elems * (8 if cfg.dtype == "f64" else 4)
     # rotate between buffer sets so that no step finds its inputs in L2
@@ -187,6 +257,8 @@ def run_ours(args):
 
     def step(s):
         ins, outs = sets[s % nsets]
+        if args.halo_exchange:
+            pdist.exchange_halo_x(ins, cfg.halo)
         L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
         if nf > 3:
             L.scalars(ins[3:], outs[3:], stream=st)
@@ -205,22 +277,26 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     n0 = L.launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * args.steps + 1)]
     with torch.cuda.stream(st):
         ev[0].record(st)
         for s in range(args.steps):
             ins, outs = sets[(args.warmup + s) % nsets]
+            if args.halo_exchange:
+                pdist.exchange_halo_x(ins, cfg.halo)
+            ev[3 * s + 1].record(st)
             L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
-            ev[2 * s + 1].record(st)
+            ev[3 * s + 2].record(st)
             if nf > 3:
                 L.scalars(ins[3:], outs[3:], stream=st)
-            ev[2 * s + 2].record(st)
+            ev[3 * s + 3].record(st)
     barrier()
     launches = L.launch_count() - n0
     plan = L.describe_plan()
     total_ms = ev[0].elapsed_time(ev[-1])
-    mom_ms = [ev[2 * s].elapsed_time(ev[2 * s + 1]) for s in range(args.steps)]
-    sca_ms = [ev[2 * s + 1].elapsed_time(ev[2 * s + 2]) for s in range(args.steps)]
+    swap_ms = [ev[3 * s].elapsed_time(ev[3 * s + 1]) for s in range(args.steps)]
+    mom_ms = [ev[3 * s + 1].elapsed_time(ev[3 * s + 2]) for s in range(args.steps)]
+    sca_ms = [ev[3 * s + 2].elapsed_time(ev[3 * s + 3]) for s in range(args.steps)]
     clocks = sampler.stop() if rank == 0 else None
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
@@ -249,6 +325,13 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     phase = L.step_times_ms()
+    # the same step with copies and kernels serialised on one stream: its phases are
+    # the "alone" times of the overlap ratio
+    L.set_overlap(False)
+    e2e_step()
+    torch.cuda.synchronize()
+    serial = L.step_times_ms()
+    L.set_overlap(True)
     if world > 1:
         t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -276,12 +359,18 @@ def run_ours(args):
     fam = {"": "tma", "auto": "tma", "tma": "tma", "march": "march", "generic": "generic"}[args.variant]
     tsuf = "double" if cfg.dtype == "f64" else "float"
     achieved = kb / (kms * 1e-3) / 1e9
+    traffic, traffic_src = args.traffic, "--traffic"
+    tuned = any((args.xchunk, args.group, args.stages, args.tile_y, args.warps, args.split))
+    if traffic is None and not tuned:
+        traffic, traffic_src = NCU_TRAFFIC.get((args.workload, f"{fam}_{kern}"), (None, None))
     roofline = {"bound": "hbm", "kernel": f"{fam}_{kern}<{tsuf}>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": args.traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
                 "best_launch_ms": float(np.min(mom_ms if kern == "momentum" else sca_ms)),
                 "frac_of_nominal_8TBs": achieved / 8000.0}
     kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
+    if args.halo_exchange:
+        kernels["halo_swap_ms"] = float(np.mean(swap_ms))
     if sca_b:
         kernels.update({"scalars_ms": sca_avg, "scalars_GBs": sca_b / (sca_avg * 1e-3) / 1e9})
 
@@ -296,7 +385,8 @@ def run_ours(args):
         "config": {"workload": args.workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz,
                    "halo": cfg.halo, "nq": cfg.nq, "fields_per_step": nf,
                    "l2": f"rotating {nsets} buffer sets ({nsets * 2 * nf * field_bytes / 1e6:.0f} MB) > 126 MB L2",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "parallelism": ("x-slab decomposition, halo swap every step" if args.halo_exchange
+                                   else ("replicas only" if world > 1 else "1 GPU")),
                    "variant": args.variant or "auto", "xchunk": args.xchunk, "group": args.group,
                    "stages": args.stages, "tile_y": args.tile_y, "warps": args.warps,
                    "split": args.split, "launch_plan": plan},
@@ -304,12 +394,101 @@ def run_ours(args):
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
                 "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
-                "phase_ms": phase, "chunks": 8},
+                "phase_ms": phase, "chunks": 8, "serial_phase_ms": serial,
+                "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / phase["total"],
+                "timing": "host wall clock around step_async + step_wait, pinned host buffers"},
         "gpu_launches": launches, "clocks": clocks,
     }
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------
+# config4: the paper's hybrid asynchronous step as the step
+# ---------------------------------------------------------------------------
+def run_hybrid(args):
+    """1024x1024x160 fp64, 3 momentum + 4 scalars in PINNED HOST memory; a step is
+    monc_adv_step_async (8 x-slab chunks H2D -> kernels -> D2H on three streams)
+    + monc_adv_step_wait.  Fields are perturbed on the host between steps
+    (BASELINE.json configs[4]), outside the timed region: the time of a step is
+    the library's device-event span first copy -> last copy, summed over steps."""
+    import torch
+    from paper_2009_12850_b200 import binding, synth
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("config4 is a single-GPU workload (one host link)")
+    torch.cuda.set_device(0)
+    cfg = workload_cfg("config4")
+    g = synth.grid(cfg.nz)
+    L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY,
+                        g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=cfg.dtype)
+    L.set_chunks(args.chunks)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    nf = len(names)
+    hin = []
+    for n in names:
+        t = torch.empty(L.shape, dtype=L.torch_dtype, pin_memory=True)
+        t.copy_(torch.from_numpy(synth.field(cfg, n)))
+        hin.append(t)
+    hout = [torch.zeros(L.shape, dtype=L.torch_dtype, pin_memory=True) for _ in names]
+
+    def step():
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+        L.step_inputs_consumed()
+        L.step_wait()
+        return L.step_times_ms()
+
+    for _ in range(max(1, min(args.warmup, 3))):
+        step()
+    sampler = ClockSampler(0, period_s=0.05)
+    sampler.start()
+    n0 = L.launch_count()
+    phases = []
+    for s_ in range(args.steps):
+        if not args.no_perturb:
+            for n, t in zip(names, hin):
+                synth.perturb(cfg, n, t.numpy(), s_ + 1)
+        phases.append(step())
+    launches = L.launch_count() - n0
+    clocks = sampler.stop()
+    L.set_overlap(False)
+    serial = step()
+    L.set_overlap(True)
+    plan = L.describe_plan()
+    tot_ms = float(np.sum([p_["total"] for p_ in phases]))
+    es = 8
+    plane_b = (cfg.ny + 2 * cfg.halo) * cfg.nz * es
+    h2d_b = nf * (cfg.nx + 2) * plane_b
+    d2h_b = nf * cfg.points * es
+    value = cfg.points * args.steps / (tot_ms * 1e-3) / 1e9
+    med = {k: float(np.median([p_[k] for p_ in phases])) for k in phases[0]}
+    peak, peak_src = peaks()
+    kb = (BYTES_PER_PT["momentum"]["f64"] + scalar_bytes_per_pt(cfg.nq, "f64")) * cfg.points
+    ach = kb / (serial["kernels"] * 1e-3) / 1e9
+    e2e = {"value": value, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b,
+           "steps": args.steps, "ms_per_step": tot_ms / args.steps, "chunks": args.chunks,
+           "h2d_GBs": h2d_b / (med["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (med["d2h"] * 1e-3) / 1e9,
+           "link_alone_GBs": {"h2d": h2d_b / (serial["h2d"] * 1e-3) / 1e9,
+                              "d2h": d2h_b / (serial["d2h"] * 1e-3) / 1e9},
+           "phase_ms_median": med, "serial_phase_ms": serial,
+           "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / med["total"]}
+    print(json.dumps({
+        "metric": "advection grid-points/sec", "value": value, "unit": "Gpts/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config4", "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz, "halo": cfg.halo,
+                   "nq": cfg.nq, "fields_per_step": nf, "chunks": args.chunks,
+                   "perturbed_each_step": not args.no_perturb,
+                   "l2": f"inputs stream from pinned host memory ({h2d_b / 1e9:.2f} GB per step) > 126 MB L2",
+                   "timing": "device events inside the library, first H2D -> last D2H, summed over steps",
+                   "launch_plan": plan},
+        "roofline": {"bound": "hbm", "kernel": "tma_momentum<double> + tma_scalars<double> per chunk",
+                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": kb,
+                     "avg_launch_ms": serial["kernels"],
+                     "note": "kernel time = sum over the 8 chunks, copies not overlapping; the step itself is host-link bound"},
+        "cpu_baseline": cpu_baseline(cfg, args), "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }))
 
 
 def cpu_baseline(cfg, args):
@@ -342,10 +521,10 @@ def cpu_baseline(cfg, args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3"])
+    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--xchunk", type=int, default=0)
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--stages", type=int, default=0)
@@ -356,12 +535,23 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--ref-planes", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--halo-exchange", action="store_true",
+                    help="N ranks advect x-slabs of ONE periodic domain of N*nx planes and swap halos over NCCL every step"
+                         " (default: independent replicas, no data-path collective)")
+    ap.add_argument("--chunks", type=int, default=8, help="config4: x-slab chunks per step")
+    ap.add_argument("--no-perturb", action="store_true", help="config4: keep the fields fixed between steps")
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel, if known")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = {"config1": 1000, "config2": 100, "config3": 200, "config4": 10}[args.workload]
+        if args.impl == "reference":
+            args.steps = 5
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "config4":
+        run_hybrid(args)
     else:
         run_ours(args)
 
