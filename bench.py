@@ -226,6 +226,8 @@ def run_ours(args):
                  warps=args.warps, split=args.split)
     if args.variant:
         L.set_variant(args.variant)
+    if args.no_pdl:
+        L.set_pdl(False)
     tdt = L.torch_dtype
     # weak scaling: every rank advects its own subdomain of the config's size
     # ("replicas only" until the halo-exchange row of SURVEY.md 8(f) is built);
@@ -277,26 +279,45 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     n0 = L.launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * args.steps + 1)]
+    # Events are recorded on the launch stream.  Momentum-only workloads: one event
+    # every `grp` launches (an event between two launches costs ~1 us of stream time
+    # and defeats the programmatic dependent launch of back-to-back kernels), so the
+    # mean launch duration is (event span) / grp.  With scalars: one event between
+    # the two kernels of a step as well.
+    split = nf > 3 or args.halo_exchange
+    grp = 1 if split else max(1, min(args.event_every, args.steps))
+    marks = []  # (kind, event)
     with torch.cuda.stream(st):
-        ev[0].record(st)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        marks.append(("start", e0))
         for s in range(args.steps):
             ins, outs = sets[(args.warmup + s) % nsets]
             if args.halo_exchange:
                 pdist.exchange_halo_x(ins, cfg.halo)
-            ev[3 * s + 1].record(st)
+                e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("swap", e))
             L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
-            ev[3 * s + 2].record(st)
+            if split or (s + 1) % grp == 0 or s + 1 == args.steps:
+                e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("mom", e))
             if nf > 3:
                 L.scalars(ins[3:], outs[3:], stream=st)
-            ev[3 * s + 3].record(st)
+                e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("sca", e))
     barrier()
     launches = L.launch_count() - n0
     plan = L.describe_plan()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    swap_ms = [ev[3 * s].elapsed_time(ev[3 * s + 1]) for s in range(args.steps)]
-    mom_ms = [ev[3 * s + 1].elapsed_time(ev[3 * s + 2]) for s in range(args.steps)]
-    sca_ms = [ev[3 * s + 2].elapsed_time(ev[3 * s + 3]) for s in range(args.steps)]
+    total_ms = marks[0][1].elapsed_time(marks[-1][1])
+    span = {"swap": 0.0, "mom": 0.0, "sca": 0.0}
+    best = {"swap": 1e30, "mom": 1e30, "sca": 1e30}
+    done = 0
+    for (k0_, a), (k1_, b) in zip(marks[:-1], marks[1:]):
+        ms = a.elapsed_time(b)
+        span[k1_] += ms
+        n_in = 1
+        if k1_ == "mom" and not split:
+            n_in = min(grp, args.steps - done)
+            done += n_in
+        best[k1_] = min(best[k1_], ms / n_in)
+    mom_avg, sca_avg, swap_avg = (span[k] / args.steps for k in ("mom", "sca", "swap"))
     clocks = sampler.stop() if rank == 0 else None
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
@@ -351,7 +372,6 @@ def run_ours(args):
     peak, peak_src = peaks()
     mom_b = BYTES_PER_PT["momentum"][cfg.dtype] * cfg.points
     sca_b = scalar_bytes_per_pt(cfg.nq, cfg.dtype) * cfg.points if cfg.nq else 0
-    mom_avg, sca_avg = float(np.mean(mom_ms)), float(np.mean(sca_ms))
     if sca_b and sca_avg > mom_avg:
         kern, kb, kms = "scalars", sca_b, sca_avg
     else:
@@ -366,11 +386,12 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": f"{fam}_{kern}<{tsuf}>", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
-                "best_launch_ms": float(np.min(mom_ms if kern == "momentum" else sca_ms)),
+                "best_launch_ms": best["mom" if kern == "momentum" else "sca"],
+                "launches_per_event": grp if kern == "momentum" else 1,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
     kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
     if args.halo_exchange:
-        kernels["halo_swap_ms"] = float(np.mean(swap_ms))
+        kernels["halo_swap_ms"] = swap_avg
     if sca_b:
         kernels.update({"scalars_ms": sca_avg, "scalars_GBs": sca_b / (sca_avg * 1e-3) / 1e9})
 
@@ -389,7 +410,7 @@ def run_ours(args):
                                    else ("replicas only" if world > 1 else "1 GPU")),
                    "variant": args.variant or "auto", "xchunk": args.xchunk, "group": args.group,
                    "stages": args.stages, "tile_y": args.tile_y, "warps": args.warps,
-                   "split": args.split, "launch_plan": plan},
+                   "split": args.split, "pdl": not args.no_pdl, "launch_plan": plan},
         "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
@@ -533,6 +554,9 @@ def main():
     ap.add_argument("--split", type=int, default=0)
     ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march", "tma"])
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--event-every", type=int, default=10,
+                    help="momentum-only workloads: launches between two timing events")
+    ap.add_argument("--no-pdl", action="store_true", help="plain stream order between kernels")
     ap.add_argument("--ref-planes", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--halo-exchange", action="store_true",

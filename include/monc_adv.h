@@ -160,6 +160,11 @@ int monc_adv_set_overlap(monc_adv_t h, int on);
 int monc_adv_set_form(monc_adv_t h, int form);
 /* 0 (default): tendencies overwritten.  1: added into the output buffers. */
 int monc_adv_set_accumulate(monc_adv_t h, int on);
+/* 1 (default): the TMA kernels are launched with CUDA's programmatic
+ * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
+ * predecessor in the stream (it waits for the predecessor's completion before
+ * touching any field: results are unchanged).  0: plain stream order. */
+int monc_adv_set_pdl(monc_adv_t h, int on);
 /* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
  * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
  * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need

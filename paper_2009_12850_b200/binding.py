@@ -29,7 +29,7 @@ SYMBOLS = [
     "monc_adv_scalars", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
     "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range",
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
-    "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_variant",
+    "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
     "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version",
 ]
@@ -76,7 +76,7 @@ def load():
     lib.monc_adv_step_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
-                 "monc_adv_set_accumulate", "monc_adv_set_variant"):
+                 "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -236,6 +236,9 @@ class MoncAdv:
 
     def set_accumulate(self, on):
         self._check(self._lib.monc_adv_set_accumulate(self._h, int(bool(on))))
+
+    def set_pdl(self, on):
+        self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
 
     def set_variant(self, variant):
         variant = {"auto": 0, "generic": 1, "march": 2, "tma": 3}.get(variant, variant)

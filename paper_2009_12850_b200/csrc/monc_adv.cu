@@ -33,7 +33,7 @@ struct monc_adv_s {
   void *d_tz[4] = {nullptr, nullptr, nullptr, nullptr};  // tzc1, tzc2, tzd1, tzd2 (dtype)
   std::vector<double> tz_host[4];                        // as stored on the device
   const void *wind[3] = {nullptr, nullptr, nullptr};
-  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0;
+  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1;
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
@@ -155,6 +155,25 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
   return pl;
 }
 
+// Launch with the programmatic stream-serialisation attribute (PDL): the kernel
+// may begin (barrier set-up, coefficient loads) while its predecessor in the
+// stream drains; it calls griddepcontrol.wait before touching any field.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(monc_adv_t h, void (*kernel)(KArgs...), dim3 grid, int threads, size_t smem,
+                       cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3((unsigned)threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = h->pdl ? 1 : 0;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <typename T>
 int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
                     int ia, int ib, cudaStream_t st) {
@@ -167,10 +186,16 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
     return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
   if (pl.ok) {
     p.xc = pl.xc;
-    CU(cudaFuncSetAttribute(tma_momentum<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     dim3 grid(pl.tiles, pl.nchunks);
-    tma_momentum<T><<<grid, pl.ty * p.wzc * 32, pl.smem, st>>>(p, pl.ty, pl.stages, u, v, w,
-                                                                     su, sv, sw);
+    if (h->accumulate) {
+      CU(cudaFuncSetAttribute(tma_momentum<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+      CU(launch_pdl(h, tma_momentum<T, true>, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages,
+                    u, v, w, su, sv, sw));
+    } else {
+      CU(cudaFuncSetAttribute(tma_momentum<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+      CU(launch_pdl(h, tma_momentum<T, false>, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages,
+                    u, v, w, su, sv, sw));
+    }
     char b[160];
     snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d threads=%d smem=%zu", pl.ty,
              pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.ty * p.wzc * 32, pl.smem);
@@ -313,9 +338,8 @@ int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps
   CU(cudaFuncSetAttribute(tma_scalars<T, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
-  tma_scalars<T, GW><<<grid, threads, pl.smem, st>>>(p, maps, outs, nq, (nq + pl.gb - 1) / pl.gb,
-                                                     pl.gb, pl.ty, pl.zw, pl.ss, pl.stages,
-                                                     pl.fieldsz);
+  CU(launch_pdl(h, tma_scalars<T, GW>, grid, threads, pl.smem, st, p, maps, outs, nq,
+                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
 }
 
@@ -822,6 +846,12 @@ int monc_adv_set_form(monc_adv_t h, int form) {
 int monc_adv_set_accumulate(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
   h->accumulate = on ? 1 : 0;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_pdl(monc_adv_t h, int on) {
+  if (!h) return MONC_ADV_EINVAL;
+  h->pdl = on ? 1 : 0;
   return MONC_ADV_OK;
 }
 

@@ -58,6 +58,17 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void *src, uint3
       : "memory");
 }
 
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic
+// stream-serialisation attribute may start while its predecessor in the stream
+// drains.  pdl_launch_dependents() lets the successor's blocks be scheduled as
+// soon as this grid's blocks have all started; pdl_wait() blocks until the
+// predecessor has completed and its writes are visible -- everything before it
+// must touch only memory no kernel writes (the coefficient tables).
+__device__ __forceinline__ void pdl_launch_dependents() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ Vec<double> lds_vec(const double *p) {
   const double2 t = *reinterpret_cast<const double2 *>(p);
   Vec<double> r;
@@ -81,13 +92,77 @@ __device__ __forceinline__ Vec<T> up_from_smem(const Vec<T> &a, const T *next) {
   return r;
 }
 
-// dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages mbarriers
+// ---------------------------------------------------------------------------
+// Shared-memory loads by 32-bit shared-window address with a compile-time byte
+// offset folded into the instruction ([R + imm]): the consumers' address
+// arithmetic is then a handful of 32-bit adds per plane.
+// ---------------------------------------------------------------------------
+template <int OFF>
+__device__ __forceinline__ Vec<double> lds_at(uint32_t a, const double *) {
+  Vec<double> r;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(r.v[0]), "=d"(r.v[1]) : "r"(a), "n"(OFF));
+  return r;
+}
+template <int OFF>
+__device__ __forceinline__ Vec<float> lds_at(uint32_t a, const float *) {
+  Vec<float> r;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+               : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "r"(a), "n"(OFF));
+  return r;
+}
+template <int OFF>
+__device__ __forceinline__ double lds1_at(uint32_t a, const double *) {
+  double r;
+  asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(r) : "r"(a), "n"(OFF));
+  return r;
+}
+template <int OFF>
+__device__ __forceinline__ float lds1_at(uint32_t a, const float *) {
+  float r;
+  asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(r) : "r"(a), "n"(OFF));
+  return r;
+}
+// r[e] = a[e+1]; the last element is the scalar `top` (level k0 + NK)
 template <typename T>
+__device__ __forceinline__ Vec<T> up_with(const Vec<T> &a, const T top) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> r;
+#pragma unroll
+  for (int e = 0; e + 1 < NK; ++e) r.v[e] = a.v[e + 1];
+  r.v[NK - 1] = top;
+  return r;
+}
+
+// values of one x plane a thread carries to the next x step: u, v, w at its
+// column and v at the column to the south
+template <typename T>
+struct PlaneRegs {
+  Vec<T> u, v, vs, w;
+};
+// the three x-face fluxes carried to the next x step
+template <typename T>
+struct XFlux {
+  Vec<T> xx, xy, xz;
+};
+
+// ---------------------------------------------------------------------------
+// tma_momentum<T, ACC>: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks
+// su/sv/sw) from a TMA-fed shared-memory ring.
+//
+// dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages
+// mbarriers.  The x loop is unrolled by two with the register sets of the
+// centre and east planes (and of the west/east x fluxes) swapping roles, so
+// the plane rotation costs no register moves.
+// ---------------------------------------------------------------------------
+template <typename T, bool ACC>
 __global__ void __launch_bounds__(kTmaThreads, 1)
 tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__restrict__ u,
              const T *__restrict__ v, const T *__restrict__ w, T *__restrict__ su,
              T *__restrict__ sv, T *__restrict__ sw) {
   constexpr int NK = VecOf<T>::NK;
+  constexpr int SZ = (int)sizeof(T);
+  constexpr int UP = NK * SZ;  // byte offset of the level above a vector's last element
+  const T *const tag = nullptr;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -112,21 +187,32 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   }
   __syncthreads();
 
+  pdl_launch_dependents();
   if (warp >= ncw) return;
+  // coefficient tables are written once at create: safe to read before pdl_wait
+  const int col = warp / p.wzc;
+  const int zc = warp - col * p.wzc;
+  const int k0r = (zc * 32 + lane) * NK;
+  const bool act = k0r < nz;
+  const int k0 = act ? k0r : nz - NK;
+  const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+  const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
+  pdl_wait();  // the fields may have been written by the previous kernel in the stream
   // ---------------- producer role: lane 0 of the last warp ----------------
   const bool producer = (warp == ncw - 1) && lane == 0;
-  const uint32_t tile_bytes = (uint32_t)((ncol + 2) * nz * (int)sizeof(T));
+  const uint32_t tile_bytes = (uint32_t)((ncol + 2) * nz * SZ);
   const uint32_t t0 = smem_u32(tiles);
+  const uint32_t fb = (uint32_t)(fieldsz * SZ), sb = 3u * fb, nzb = (uint32_t)(nz * SZ);
   long long g_next = ((long long)(i0 - 1) * p.nyh + (jr0 + p.h - 1)) * nz;  // next plane to load
   int pl_next = 0, s_next = 0;
   uint32_t par_next = 0;  // parity of the empty-phase the next refill of slot s_next waits for
   auto issue_plane = [&]() {
     const uint32_t full = bar0 + 8 * s_next;
     mbar_expect_tx(full, 3 * tile_bytes);
-    const uint32_t dst = t0 + (uint32_t)(s_next * stagesz * (int)sizeof(T));
+    const uint32_t dst = t0 + (uint32_t)s_next * sb;
     tma_load_1d(dst, u + g_next, tile_bytes, full);
-    tma_load_1d(dst + (uint32_t)(fieldsz * (int)sizeof(T)), v + g_next, tile_bytes, full);
-    tma_load_1d(dst + (uint32_t)(2 * fieldsz * (int)sizeof(T)), w + g_next, tile_bytes, full);
+    tma_load_1d(dst + fb, v + g_next, tile_bytes, full);
+    tma_load_1d(dst + 2 * fb, w + g_next, tile_bytes, full);
     g_next += p.plane;
     ++pl_next;
     if (++s_next == nstages) s_next = 0;
@@ -137,54 +223,82 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   }
 
   // ---------------- consumers: warp <-> (column, z chunk) ----------------
-  const int col = warp / p.wzc;
-  const int zc = warp - col * p.wzc;
-  const int k0r = (zc * 32 + lane) * NK;
-  const bool act = k0r < nz;
-  const int k0 = act ? k0r : nz - NK;
   const bool bot_edge = act && lane == 0 && zc > 0;
-  const int e0 = (col + 1) * nz + k0;  // element index inside a field tile
-  const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
-  const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
+  const bool first_level = k0 == 0;        // element 0 is level K = 1: no tendency
+  const bool last_level = k0 + NK == nz;   // element NK-1 is level K = nz: sw = 0
   const T cx = p.cx, cy = p.cy;
   const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
   T *qu = su + c0, *qv = sv + c0, *qw = sw + c0;
+  const long long plane = p.plane;
+  const uint32_t a0 = t0 + (uint32_t)(((col + 1) * nz + k0) * SZ);  // u(column, k0) in stage 0
 
   mbar_wait(bar0, 0);  // plane i0-1
-  const T *A = tiles;
-  Vec<T> uC = lds_vec(A + e0), vC = lds_vec(A + fieldsz + e0);
-  Vec<T> vS = lds_vec(A + fieldsz + e0 - nz), wC = lds_vec(A + 2 * fieldsz + e0);
-  Vec<T> fxx_w, fxy_w, fxz_w;
+  PlaneRegs<T> RA, RB;
+  XFlux<T> FA, FB;
+  RA.u = lds_at<0>(a0, tag);
+  RA.v = lds_at<0>(a0 + fb, tag);
+  RA.vs = lds_at<0>(a0 + fb - nzb, tag);
+  RA.w = lds_at<0>(a0 + 2 * fb, tag);
 #pragma unroll
-  for (int e = 0; e < NK; ++e) fxx_w.v[e] = fxy_w.v[e] = fxz_w.v[e] = T(0);
+  for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
 
   int sC = 0, sE = 1 % nstages;
   uint32_t parE = (nstages == 1) ? 1 : 0;
-#pragma unroll 1
-  for (int t = 0; t < nsteps; ++t) {
+  uint32_t pC = a0, pE = a0 + (uint32_t)sE * sb;
+  int t = 0;
+
+  // one x step: centre plane in RC (registers) / stage sC, east plane arriving in stage sE
+  auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
     mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
-    const T *B = tiles + sE * stagesz;
-    A = tiles + sC * stagesz;
-    const T *Au = A + e0, *Av = A + fieldsz + e0, *Aw = A + 2 * fieldsz + e0;
-    const Vec<T> uS = lds_vec(Au - nz), uN = lds_vec(Au + nz);
-    const Vec<T> vN = lds_vec(Av + nz);
-    const Vec<T> wS = lds_vec(Aw - nz), wN = lds_vec(Aw + nz);
-    const Vec<T> uE = lds_vec(B + e0), vE = lds_vec(B + fieldsz + e0);
-    const Vec<T> vSE = lds_vec(B + fieldsz + e0 - nz), wE = lds_vec(B + 2 * fieldsz + e0);
-    const Vec<T> uCu = up_from_smem(uC, Au + NK), vCu = up_from_smem(vC, Av + NK);
-    const Vec<T> wCu = up_from_smem(wC, Aw + NK), vSu = up_from_smem(vS, Av - nz + NK);
+    const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
+    const uint32_t pCuS = pC - nzb, pCvS = pCv - nzb, pCwS = pCw - nzb;
+    const Vec<T> uS = lds_at<0>(pCuS, tag), uN = lds_at<0>(pC + nzb, tag);
+    const Vec<T> vN = lds_at<0>(pCv + nzb, tag);
+    const Vec<T> wS = lds_at<0>(pCwS, tag), wN = lds_at<0>(pCw + nzb, tag);
+    RE.u = lds_at<0>(pE, tag);
+    RE.v = lds_at<0>(pEv, tag);
+    RE.vs = lds_at<0>(pEv - nzb, tag);
+    RE.w = lds_at<0>(pEv + fb, tag);
+    const Vec<T> uCu = up_with(RC.u, lds1_at<UP>(pC, tag)), vCu = up_with(RC.v, lds1_at<UP>(pCv, tag));
+    const Vec<T> wCu = up_with(RC.w, lds1_at<UP>(pCw, tag)), vSu = up_with(RC.vs, lds1_at<UP>(pCvS, tag));
     T b_xz = T(0), b_yz = T(0), b_zz = T(0);
-    if (bot_edge) {
-      const T ub = Au[-1], vb = Av[-1], wb = Aw[-1];
-      const T web = B[2 * fieldsz + e0 - 1], wnb = Aw[nz - 1];
-      b_xz = (ub + uC.v[0]) * (wb + web);
-      b_yz = (vb + vC.v[0]) * (wb + wnb);
-      b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+    if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
+      const T ub = lds1_at<-SZ>(pC, tag), vb = lds1_at<-SZ>(pCv, tag), wb = lds1_at<-SZ>(pCw, tag);
+      const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + nzb, tag);
+      b_xz = (ub + RC.u.v[0]) * (wb + web);
+      b_yz = (vb + RC.v.v[0]) * (wb + wnb);
+      b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
     }
+    // six distinct face fluxes (see momentum_step)
+    Vec<T> fyz_n, fzz_t, ry, rv, rwy;
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      const T a = RC.u.v[e] + RE.u.v[e];
+      FE.xx.v[e] = a * a;
+      FE.xy.v[e] = (RC.u.v[e] + uN.v[e]) * (RC.v.v[e] + RE.v.v[e]);
+      const T fxy_se = (uS.v[e] + RC.u.v[e]) * (RC.vs.v[e] + RE.vs.v[e]);
+      FE.xz.v[e] = (RC.u.v[e] + uCu.v[e]) * (RC.w.v[e] + RE.w.v[e]);
+      const T bn = RC.v.v[e] + vN.v[e], bs = RC.vs.v[e] + RC.v.v[e];
+      fyz_n.v[e] = (RC.v.v[e] + vCu.v[e]) * (RC.w.v[e] + wN.v[e]);
+      const T fyz_s = (RC.vs.v[e] + vSu.v[e]) * (wS.v[e] + RC.w.v[e]);
+      const T g = RC.w.v[e] + wCu.v[e];
+      fzz_t.v[e] = g * g;
+      ry.v[e] = cy * (fxy_se - FE.xy.v[e]);
+      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);
+      rv.v[e] = cx * (FW.xy.v[e] - FE.xy.v[e]) + cy * (bs * bs - bn * bn);
+    }
+    const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
+    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
+    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
     Vec<T> ou, ov, ow;
-    momentum_step<T>(cx, cy, c1, c2, d1, d2, uC, vC, vS, wC, uS, uN, vN, wS, wN, uE, vE, vSE, wE,
-                     uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, lane, k0, nz, fxx_w, fxy_w, fxz_w, ou,
-                     ov, ow);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
+      ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
+      ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+    }
+    if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
+    if (last_level) ow.v[NK - 1] = T(0);
     // this warp is done with plane i's slot
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
@@ -196,18 +310,27 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     }
     if (t > 0) {
       if (act) {
-        if (p.accumulate) {
+        if (ACC) {
           const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
 #pragma unroll
           for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
         }
         st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
       }
-      qu += p.plane; qv += p.plane; qw += p.plane;
+      qu += plane; qv += plane; qw += plane;
     }
-    uC = uE; vC = vE; vS = vSE; wC = wE;
     sC = sE;
-    if (++sE == nstages) { sE = 0; parE ^= 1; }
+    pC = pE;
+    pE += sb;
+    if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
+    ++t;
+  };
+#pragma unroll 1
+  while (true) {
+    step(RA, RB, FA, FB);
+    if (t == nsteps) break;
+    step(RB, RA, FB, FA);
+    if (t == nsteps) break;
   }
 }
 
@@ -319,12 +442,14 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   }
   __syncthreads();
 
+  pdl_launch_dependents();
   if (warp == nwarps_c) {
     // ---------------- producer warp: one lane per field ----------------
     const int nfld = 3 + cnt;
     const uint32_t box_bytes = (uint32_t)(rows * RS * (int)sizeof(T));
     const CUtensorMap *mymap = &maps.m[lane < 3 ? lane : 3 + s0 + min(lane - 3, cnt - 1)];
     if (lane < nfld) prefetch_tensormap(mymap);
+    pdl_wait();  // the fields may have been written by the previous kernel in the stream
     const uint32_t t0 = smem_u32(tiles);
     int s = 0;
     uint32_t par = 1;  // a fresh mbarrier passes a wait on parity 1: the first lap does not block
@@ -360,6 +485,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
   const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
   long long c = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+  pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
 
   Vec<T> uP, qP[GW], fxP[GW], P[GW];  // carried from the previous plane
 #pragma unroll
