@@ -142,8 +142,9 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
       const long waves = (blocks + h->sm_count - 1) / h->sm_count;
-      // time ~ waves * (columns per block) * (planes per block + ramp-up planes)
-      const double cost = (double)waves * ty * (xc + 3) * (1.0 + 0.02 * (tymax - ty));
+      // time ~ waves * (columns per block + the L2/shared-memory cost of its two halo
+      // columns) * (planes per block + ramp-up planes)
+      const double cost = (double)waves * (ty + 0.7) * (xc + 3) * (1.0 + 0.02 * (tymax - ty));
       if (cost < best) {
         best = cost;
         pl.ok = true; pl.ty = ty; pl.stages = S; pl.xc = xc; pl.tiles = tiles;
@@ -279,8 +280,8 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
   // Cost model, calibrated on B200:
   // a block step (one plane) takes max(DRAM time of its bytes at this SM's share
   // of HBM bandwidth, the serial time of one warp's gw scalars), stretched when
-  // the ring is shallow, plus a fixed synchronisation cost; a launch takes
-  // waves * (planes per block + 2) steps.
+  // the ring has only two stages, plus a fixed synchronisation cost; a launch takes
+  // waves * (planes per block + 4) steps.
   const double sm_gbs = 6200.0 / h->sm_count;
   for (int gb = std::min(n, 10); gb >= 1; --gb) {
     if (h->group > 0 && gb != std::min(h->group, std::min(n, 10))) continue;
@@ -304,10 +305,12 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
           if (h->stages > 0) S = std::min(S, h->stages);
           if (S < 2) continue;
           const int tiles = ((h->ny + ty - 1) / ty) * nzt * ngroups;
-          const double dram_b = ((3.0 / ngroups + gb) + gb) * ty * ZB * sizeof(T);  // wind shared via L2
+          // the groups after the first re-read the wind; about half of that hits L2
+          const double wind = 3.0 * (1.0 + 0.5 * (ngroups - 1)) / ngroups;
+          const double dram_b = ((wind + gb) + gb) * ty * ZB * sizeof(T);
           const double t_mem = dram_b / (sm_gbs * 1e3);                            // us
-          const double t_warp = 0.15 + 0.30 * gw;                                    // us
-          const double shallow = S >= 5 ? 1.0 : (S == 4 ? 1.10 : (S == 3 ? 1.15 : 1.5));
+          const double t_warp = 0.15 + 0.25 * gw;                                    // us
+          const double shallow = S >= 3 ? 1.0 : 1.15;
           const double t_step = std::max(t_mem, t_warp) * shallow + 0.05;
           const int nch_lo = nch_fixed ? nch_fixed : 1;
           const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 8);
@@ -315,7 +318,7 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
             const int xc = (nplanes + nch - 1) / nch;
             const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
             const long waves = (blocks + h->sm_count - 1) / h->sm_count;
-            const double cost = (double)waves * (xc + 2) * t_step;
+            const double cost = (double)waves * (xc + 4) * t_step;  // +2 halo planes, ~2 steps of start-up latency
             if (cost < best) {
               best = cost;
               pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
@@ -332,15 +335,22 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
   return pl;
 }
 
+template <typename T, int GW, bool ACC>
+int launch_tma_scalars_acc(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
+                           const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+  dim3 grid(pl.tiles, pl.nchunks);
+  const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC>, grid, threads, pl.smem, st, p, maps, outs, nq,
+                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
+  return MONC_ADV_OK;
+}
+
 template <typename T, int GW>
 int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
                        const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(cudaFuncSetAttribute(tma_scalars<T, GW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-  dim3 grid(pl.tiles, pl.nchunks);
-  const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW>, grid, threads, pl.smem, st, p, maps, outs, nq,
-                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
-  return MONC_ADV_OK;
+  return h->accumulate ? launch_tma_scalars_acc<T, GW, true>(h, p, maps, outs, nq, pl, st)
+                       : launch_tma_scalars_acc<T, GW, false>(h, p, maps, outs, nq, pl, st);
 }
 
 // One launch of tma_scalars per kMaxScalarsPerLaunch scalars.  *done = false

@@ -397,7 +397,7 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 constexpr int kScalarConsumerWarps = 15;
 constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
 
-template <typename T, int GW>
+template <typename T, int GW, bool ACC>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const int nq, const int ngroups, const int gb, const int ty, const int zw,
@@ -487,37 +487,50 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   long long c = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
   pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
 
-  Vec<T> uP, qP[GW], fxP[GW], P[GW];  // carried from the previous plane
+  // carried from the previous plane, per scalar: q, the x flux through its west
+  // face and the y + z part of its tendency.  (Swapping two register sets in an
+  // x loop unrolled by two, as tma_momentum does, spills here: measured slower.)
+  struct Carry { Vec<T> q, fx, P; };
+  Carry CA[GW], CB[GW];
+  Vec<T> uA, uB;
 #pragma unroll
-  for (int e = 0; e < NK; ++e) uP.v[e] = T(0);
+  for (int e = 0; e < NK; ++e) uA.v[e] = T(0);
 #pragma unroll
   for (int s = 0; s < GW; ++s) {
 #pragma unroll
-    for (int e = 0; e < NK; ++e) qP[s].v[e] = fxP[s].v[e] = P[s].v[e] = T(0);
+    for (int e = 0; e < NK; ++e) CA[s].q.v[e] = CA[s].fx.v[e] = CA[s].P.v[e] = T(0);
   }
+  constexpr int SZ = (int)sizeof(T);
+  constexpr int UP = NK * SZ;
+  const T *const tag = nullptr;
+  const bool first_level = k0 == 0;  // element 0 is level K = 1: no tendency
+  const uint32_t fb = (uint32_t)(fieldsz * SZ), sbytes = (uint32_t)(stagesz * SZ), rsb = (uint32_t)(RS * SZ);
+  const uint32_t a0 = smem_u32(tiles) + (uint32_t)(e0 * SZ);   // u(column, k0) in stage 0
+  const uint32_t q0off = (uint32_t)(3 + sb) * fb;              // this warp's first scalar
+  const long long plane = p.plane;
 
-  int st = 0;
+  int st = 0, t = 0;
   uint32_t par = 0;
-#pragma unroll 1
-  for (int t = 0; t < nplanes; ++t) {
+  uint32_t pA = a0;
+  auto step = [&](const Carry (&CP)[GW], Carry (&CN)[GW], const Vec<T> &uP, Vec<T> &uN) {
     mbar_wait(bar0 + 8 * st, par);  // plane i0-1+t has landed
-    const T *A = tiles + st * stagesz + e0;
-    const Vec<T> uC = lds_vec(A), vC = lds_vec(A + fieldsz);
-    const Vec<T> vS = lds_vec(A + fieldsz - RS), wC = lds_vec(A + 2 * fieldsz);
-    const T wb = bot_edge ? A[2 * fieldsz - 1] : T(0);
+    const uint32_t pV = pA + fb, pW = pV + fb;
+    uN = lds_at<0>(pA, tag);
+    const Vec<T> vC = lds_at<0>(pV, tag), vS = lds_at<0>(pV - rsb, tag), wC = lds_at<0>(pW, tag);
+    const T wb = bot_edge ? lds1_at<-SZ>(pW, tag) : T(0);
     const bool store = act && t >= 2;
+    uint32_t pQ = pA + q0off;
 #pragma unroll
     for (int s = 0; s < GW; ++s) {
       if (s < mycnt) {  // warp-uniform
-        const T *Aq = A + (3 + sb + s) * fieldsz;
-        const Vec<T> q = lds_vec(Aq);
-        const Vec<T> qS = lds_vec(Aq - RS), qN = lds_vec(Aq + RS);
-        const Vec<T> qU = up_from_smem(q, Aq + NK);
-        const T b_z = bot_edge ? wb * (Aq[-1] + q.v[0]) : T(0);
-        Vec<T> fx, fz_t, hy;
+        const Vec<T> q = lds_at<0>(pQ, tag);
+        const Vec<T> qS = lds_at<0>(pQ - rsb, tag), qN = lds_at<0>(pQ + rsb, tag);
+        const Vec<T> qU = up_with(q, lds1_at<UP>(pQ, tag));
+        const T b_z = bot_edge ? wb * (lds1_at<-SZ>(pQ, tag) + q.v[0]) : T(0);
+        Vec<T> fz_t, hy;
 #pragma unroll
         for (int e = 0; e < NK; ++e) {
-          fx.v[e] = uP.v[e] * (qP[s].v[e] + q.v[e]);  // face between planes i-1 and i
+          CN[s].fx.v[e] = uP.v[e] * (CP[s].q.v[e] + q.v[e]);  // face between planes i-1 and i
           hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + q.v[e]) - vC.v[e] * (q.v[e] + qN.v[e]));
           fz_t.v[e] = wC.v[e] * (q.v[e] + qU.v[e]);
         }
@@ -525,13 +538,10 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
         if (store) {  // sq of plane i-1 is complete
           Vec<T> o;
 #pragma unroll
-          for (int e = 0; e < NK; ++e) {
-            T x = P[s].v[e] + cx2 * (fxP[s].v[e] - fx.v[e]);
-            if (k0 + e == 0) x = T(0);
-            o.v[e] = x;
-          }
-          T *sq = outs.sq[s0 + sb + s] + c;
-          if (p.accumulate) {
+          for (int e = 0; e < NK; ++e) o.v[e] = CP[s].P.v[e] + cx2 * (CP[s].fx.v[e] - CN[s].fx.v[e]);
+          if (first_level) o.v[0] = T(0);
+          T *sq = outs.sq[s0 + sb + s] + c;  // pointer table lives in the constant bank
+          if (ACC) {
             const Vec<T> a = ld_vec_rw(sq);
 #pragma unroll
             for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
@@ -540,17 +550,25 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
         }
 #pragma unroll
         for (int e = 0; e < NK; ++e)
-          P[s].v[e] = hy.v[e] + (c1.v[e] * fz_b.v[e] - c2.v[e] * fz_t.v[e]);
-        qP[s] = q;
-        fxP[s] = fx;
+          CN[s].P.v[e] = hy.v[e] + (c1.v[e] * fz_b.v[e] - c2.v[e] * fz_t.v[e]);
+        CN[s].q = q;
+        pQ += fb;
       }
     }
-    uP = uC;
     // this warp is done with the slot
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
-    if (t >= 2) c += p.plane;
-    if (++st == nstages) { st = 0; par ^= 1; }
+    if (t >= 2) c += plane;
+    pA += sbytes;
+    if (++st == nstages) { st = 0; par ^= 1; pA = a0; }
+    ++t;
+  };
+#pragma unroll 1
+  while (t < nplanes) {
+    step(CA, CB, uA, uB);
+    uA = uB;
+#pragma unroll
+    for (int s = 0; s < GW; ++s) CA[s] = CB[s];
   }
 }
 
