@@ -12,6 +12,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -181,22 +182,21 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
   if (ib <= ia) return MONC_ADV_OK;
   KParams<T> p = make_params<T>(h, ia, ib);
   TmaPlan pl;
-  if ((h->variant == 3 || h->variant == 0) && h->form == MONC_ADV_FORM_FLUX)
-    pl = plan_tma<T>(h, ib - ia, 3);
+  if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia, 3);
   if (h->variant == 3 && !pl.ok)
     return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
   if (pl.ok) {
     p.xc = pl.xc;
     dim3 grid(pl.tiles, pl.nchunks);
-    if (h->accumulate) {
-      CU(cudaFuncSetAttribute(tma_momentum<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-      CU(launch_pdl(h, tma_momentum<T, true>, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages,
-                    u, v, w, su, sv, sw));
-    } else {
-      CU(cudaFuncSetAttribute(tma_momentum<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-      CU(launch_pdl(h, tma_momentum<T, false>, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages,
-                    u, v, w, su, sv, sw));
-    }
+    auto go = [&](auto kernel) -> int {
+      CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+      CU(launch_pdl(h, kernel, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages, u, v, w, su, sv, sw));
+      return MONC_ADV_OK;
+    };
+    const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
+    const int rc = h->accumulate ? (skew ? go(tma_momentum<T, true, true>) : go(tma_momentum<T, true, false>))
+                                 : (skew ? go(tma_momentum<T, false, true>) : go(tma_momentum<T, false, false>));
+    if (rc != MONC_ADV_OK) return rc;
     char b[160];
     snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d threads=%d smem=%zu", pl.ty,
              pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.ty * p.wzc * 32, pl.smem);
@@ -252,9 +252,14 @@ bool encode_field_map(monc_adv_t h, CUtensorMap *m, const void *base, int box_z,
   const cuuint32_t estr[3] = {1u, 1u, 1u};
   const CUtensorMapDataType dt =
       sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  static const int promo = []() { const char *e = getenv("MONC_ADV_L2PROMO"); return e ? atoi(e) : 3; }();
+  const CUtensorMapL2promotion pr = promo == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
+                                  : promo == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+                                  : promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                               : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
   return enc(m, dt, 3, const_cast<void *>(base), gdim, gstr, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+             pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // geometry of tma_scalars: ty columns x zw z-chunks (32 vectors each) x ss
@@ -335,13 +340,13 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
   return pl;
 }
 
-template <typename T, int GW, bool ACC>
-int launch_tma_scalars_acc(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
-                           const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+template <typename T, int GW, bool ACC, bool SKEW>
+int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
+                         const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC, SKEW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW, ACC>, grid, threads, pl.smem, st, p, maps, outs, nq,
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW>, grid, threads, pl.smem, st, p, maps, outs, nq,
                 (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
 }
@@ -349,8 +354,12 @@ int launch_tma_scalars_acc(monc_adv_t h, const KParams<T> &p, const TensorMaps &
 template <typename T, int GW>
 int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
                        const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  return h->accumulate ? launch_tma_scalars_acc<T, GW, true>(h, p, maps, outs, nq, pl, st)
-                       : launch_tma_scalars_acc<T, GW, false>(h, p, maps, outs, nq, pl, st);
+  const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
+  if (h->accumulate)
+    return skew ? launch_tma_scalars_k<T, GW, true, true>(h, p, maps, outs, nq, pl, st)
+                : launch_tma_scalars_k<T, GW, true, false>(h, p, maps, outs, nq, pl, st);
+  return skew ? launch_tma_scalars_k<T, GW, false, true>(h, p, maps, outs, nq, pl, st)
+              : launch_tma_scalars_k<T, GW, false, false>(h, p, maps, outs, nq, pl, st);
 }
 
 // One launch of tma_scalars per kMaxScalarsPerLaunch scalars.  *done = false
@@ -419,7 +428,7 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
     ptrs.q[n] = (const T *)q[n < nq ? n : 0];
     ptrs.sq[n] = (T *)sq[n < nq ? n : 0];
   }
-  if ((h->variant == 3 || h->variant == 0) && h->form == MONC_ADV_FORM_FLUX) {
+  if (h->variant == 3 || h->variant == 0) {
     bool done = false;
     const int rc = run_tma_scalars<T>(h, p, u, v, w, q, sq, nq, ia, ib, st, &done);
     if (rc != MONC_ADV_OK || done) return rc;

@@ -154,7 +154,7 @@ struct XFlux {
 // centre and east planes (and of the west/east x fluxes) swapping roles, so
 // the plane rotation costs no register moves.
 // ---------------------------------------------------------------------------
-template <typename T, bool ACC>
+template <typename T, bool ACC, bool SKEW>
 __global__ void __launch_bounds__(kTmaThreads, 1)
 tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__restrict__ u,
              const T *__restrict__ v, const T *__restrict__ w, T *__restrict__ su,
@@ -265,10 +265,54 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
       const T ub = lds1_at<-SZ>(pC, tag), vb = lds1_at<-SZ>(pCv, tag), wb = lds1_at<-SZ>(pCw, tag);
       const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + nzb, tag);
-      b_xz = (ub + RC.u.v[0]) * (wb + web);
-      b_yz = (vb + RC.v.v[0]) * (wb + wnb);
-      b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
+      if (SKEW) {
+        b_xz = ub * (wb + web);
+        b_yz = vb * (wb + wnb);
+        b_zz = wb * (wb + RC.w.v[0]);
+      } else {
+        b_xz = (ub + RC.u.v[0]) * (wb + web);
+        b_yz = (vb + RC.v.v[0]) * (wb + wnb);
+        b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
+      }
     }
+    Vec<T> ou, ov, ow;
+    if (SKEW) {
+      // Piacsek-Williams skew form (R4): the advected parenthesis holds the
+      // neighbour's value only, so a face carries two products, A*phi_far for the
+      // point on this side and A*phi_near for the point across the face (handed on
+      // through FE in x, by shuffle in z), with the advecting sums A shared.
+      Vec<T> su_t, sv_t, sw_t, pu_t, pv_t, pw_t, ry, rv, rwy;
+#pragma unroll
+      for (int e = 0; e < NK; ++e) {
+        const T axu = RC.u.v[e] + RE.u.v[e];     // advects u through the east face
+        const T axv = RC.u.v[e] + uN.v[e];       // advects v through the east face
+        const T axw = RC.u.v[e] + uCu.v[e];      // advects w through the east face
+        const T ayu_n = RC.v.v[e] + RE.v.v[e], ayu_s = RC.vs.v[e] + RE.vs.v[e];
+        const T ayv_n = RC.v.v[e] + vN.v[e], ayv_s = RC.vs.v[e] + RC.v.v[e];
+        const T ayw_n = RC.v.v[e] + vCu.v[e], ayw_s = RC.vs.v[e] + vSu.v[e];
+        const T azu = RC.w.v[e] + RE.w.v[e];     // advects u through the top face
+        const T azv = RC.w.v[e] + wN.v[e];
+        const T azw = RC.w.v[e] + wCu.v[e];
+        ry.v[e] = cx * (FW.xx.v[e] - axu * RE.u.v[e]) + cy * (ayu_s * uS.v[e] - ayu_n * uN.v[e]);
+        rv.v[e] = cx * (FW.xy.v[e] - axv * RE.v.v[e]) + cy * (ayv_s * RC.vs.v[e] - ayv_n * vN.v[e]);
+        rwy.v[e] = cx * (FW.xz.v[e] - axw * RE.w.v[e]) + cy * (ayw_s * wS.v[e] - ayw_n * wN.v[e]);
+        FE.xx.v[e] = axu * RC.u.v[e];
+        FE.xy.v[e] = axv * RC.v.v[e];
+        FE.xz.v[e] = axw * RC.w.v[e];
+        su_t.v[e] = azu * uCu.v[e]; pu_t.v[e] = azu * RC.u.v[e];
+        sv_t.v[e] = azv * vCu.v[e]; pv_t.v[e] = azv * RC.v.v[e];
+        sw_t.v[e] = azw * wCu.v[e]; pw_t.v[e] = azw * RC.w.v[e];
+      }
+      const Vec<T> fu_b = shift_down(pu_t, lane, b_xz);
+      const Vec<T> fv_b = shift_down(pv_t, lane, b_yz);
+      const Vec<T> fw_b = shift_down(pw_t, lane, b_zz);
+#pragma unroll
+      for (int e = 0; e < NK; ++e) {
+        ou.v[e] = ry.v[e] + (c1.v[e] * fu_b.v[e] - c2.v[e] * su_t.v[e]);
+        ov.v[e] = rv.v[e] + (c1.v[e] * fv_b.v[e] - c2.v[e] * sv_t.v[e]);
+        ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
+      }
+    } else {
     // six distinct face fluxes (see momentum_step)
     Vec<T> fyz_n, fzz_t, ry, rv, rwy;
 #pragma unroll
@@ -290,12 +334,12 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
     const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
     const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
-    Vec<T> ou, ov, ow;
 #pragma unroll
     for (int e = 0; e < NK; ++e) {
       ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
       ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
       ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+    }
     }
     if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
     if (last_level) ow.v[NK - 1] = T(0);
@@ -397,7 +441,7 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 constexpr int kScalarConsumerWarps = 15;
 constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
 
-template <typename T, int GW, bool ACC>
+template <typename T, int GW, bool ACC, bool SKEW>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const int nq, const int ngroups, const int gb, const int ty, const int zw,
@@ -526,19 +570,33 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
         const Vec<T> q = lds_at<0>(pQ, tag);
         const Vec<T> qS = lds_at<0>(pQ - rsb, tag), qN = lds_at<0>(pQ + rsb, tag);
         const Vec<T> qU = up_with(q, lds1_at<UP>(pQ, tag));
-        const T b_z = bot_edge ? wb * (lds1_at<-SZ>(pQ, tag) + q.v[0]) : T(0);
-        Vec<T> fz_t, hy;
+        // SKEW (Piacsek-Williams skew form, R4): the advected parenthesis
+        // holds the far value only, so a face carries two products: the one of
+        // the point across the face is handed on (fx in x, the shuffle in z).
+        const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
+        const T b_z = SKEW ? wb * qb : wb * (qb + q.v[0]);
+        Vec<T> fz_t, fz_p, hy, fx_e;
 #pragma unroll
         for (int e = 0; e < NK; ++e) {
-          CN[s].fx.v[e] = uP.v[e] * (CP[s].q.v[e] + q.v[e]);  // face between planes i-1 and i
-          hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + q.v[e]) - vC.v[e] * (q.v[e] + qN.v[e]));
-          fz_t.v[e] = wC.v[e] * (q.v[e] + qU.v[e]);
+          if (SKEW) {
+            fx_e.v[e] = uP.v[e] * q.v[e];            // east face of plane i-1, seen from i-1
+            CN[s].fx.v[e] = uP.v[e] * CP[s].q.v[e];  // the same face seen from plane i
+            hy.v[e] = cy2 * (vS.v[e] * qS.v[e] - vC.v[e] * qN.v[e]);
+            fz_t.v[e] = wC.v[e] * qU.v[e];
+            fz_p.v[e] = wC.v[e] * q.v[e];
+          } else {
+            CN[s].fx.v[e] = uP.v[e] * (CP[s].q.v[e] + q.v[e]);  // face between planes i-1 and i
+            fx_e.v[e] = CN[s].fx.v[e];
+            hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + q.v[e]) - vC.v[e] * (q.v[e] + qN.v[e]));
+            fz_t.v[e] = wC.v[e] * (q.v[e] + qU.v[e]);
+            fz_p.v[e] = fz_t.v[e];
+          }
         }
-        const Vec<T> fz_b = shift_down(fz_t, lane, b_z);
+        const Vec<T> fz_b = shift_down(fz_p, lane, b_z);
         if (store) {  // sq of plane i-1 is complete
           Vec<T> o;
 #pragma unroll
-          for (int e = 0; e < NK; ++e) o.v[e] = CP[s].P.v[e] + cx2 * (CP[s].fx.v[e] - CN[s].fx.v[e]);
+          for (int e = 0; e < NK; ++e) o.v[e] = CP[s].P.v[e] + cx2 * (CP[s].fx.v[e] - fx_e.v[e]);
           if (first_level) o.v[0] = T(0);
           T *sq = outs.sq[s0 + sb + s] + c;  // pointer table lives in the constant bank
           if (ACC) {

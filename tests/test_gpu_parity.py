@@ -270,10 +270,49 @@ def test_scalars_need_wind_and_wind_binding_equivalence():
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_pw_skew_form(dtype):
+@pytest.mark.parametrize("variant", ["tma", "generic"])
+def test_pw_skew_form(dtype, variant):
+    # NEXT-1 (R4): the Piacsek-Williams skew form on the fast kernels;
+    # several y tiles, z chunks and x chunks with ragged tails
     cfg = gc.custom_cfg(10, 9, 40, dtype=dtype, cid=304)
-    run_momentum(cfg, form="pw_skew")
-    run_scalars(cfg, 2, form="pw_skew")
+    run_momentum(cfg, variant=variant, form="pw_skew")
+    run_scalars(cfg, 2, variant=variant, form="pw_skew")
+    cfg = gc.custom_cfg(21, 19, 200, dtype=dtype, cid=306)
+    run_momentum(cfg, variant=variant, form="pw_skew", xchunk=8)
+    run_scalars(cfg, 7, variant=variant, form="pw_skew", xchunk=8)
+
+
+def test_pw_skew_accumulate_and_P7_sums():
+    # skew + accumulate on the TMA kernels, and the exact skew checksums of the
+    # worked example (tests/golden/p7_worked_example.txt, rows "skewsum")
+    from test_oracle_pins import p7_problem, read_golden
+    P, (U, V, W, Q) = p7_problem()
+    dz = np.array([1, 1, 2, 2, 4, 4], float)
+    L = binding.MoncAdv(4, 4, 6, 2, 2.0, 4.0, dz, dz, np.array([1, 1, .5, .5, .25, .25]),
+                        np.array([2, 1, 1, .5, .5, .25]), dtype="f64")
+    L.set_variant("tma")
+    L.set_form("pw_skew")
+    d = [gc.to_dev(a, L) for a in (U, V, W, Q)]
+    outs = gc.fresh_out(L, 4)
+    L.momentum(d[0], d[1], d[2], *outs[:3])
+    L.scalars([d[3]], [outs[3]])
+    torch.cuda.synchronize()
+    assert "tma_momentum" in L.describe_plan() and "tma_scalars" in L.describe_plan()
+    res = {k: o.cpu().numpy()[2:6, 2:6] for k, o in zip(("su", "sv", "sw", "sq"), outs)}
+    n = 0
+    for r in read_golden():
+        if r[0] == "skewsum":
+            assert res[r[2]].sum() == float(Fraction(r[3])), r
+            assert np.abs(res[r[2]]).max() == float(Fraction(r[4])), r
+            n += 1
+    assert n == 4
+    L.set_accumulate(True)
+    L.momentum(d[0], d[1], d[2], *outs[:3])
+    L.scalars([d[3]], [outs[3]])
+    torch.cuda.synchronize()
+    for k, o in zip(("su", "sv", "sw", "sq"), outs):
+        assert np.array_equal(o.cpu().numpy()[2:6, 2:6], 2.0 * res[k]), k
+    L.close()
 
 
 def test_translation_invariance_bitwise_on_gpu():
