@@ -12,7 +12,6 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -142,10 +141,15 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
     for (int nch = nch_lo; nch <= nch_hi; ++nch) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
-      const long waves = (blocks + h->sm_count - 1) / h->sm_count;
+      // few blocks per SM run in lock-step waves; many are balanced dynamically
+      const double waves = blocks <= 6L * h->sm_count
+                               ? (double)((blocks + h->sm_count - 1) / h->sm_count)
+                               : (double)blocks / h->sm_count;
       // time ~ waves * (columns per block + the L2/shared-memory cost of its two halo
-      // columns) * (planes per block + ramp-up planes)
-      const double cost = (double)waves * (ty + 0.7) * (xc + 3) * (1.0 + 0.02 * (tymax - ty));
+      // columns) * (planes per block + ramp-up planes) * (long marches: SMs get unequal
+      // shares of HBM and y neighbours drift apart, measured +11 % from 32 to 64 planes)
+      const double march = 1.0 + 0.12 * std::min(xc, 64) / 32.0;
+      const double cost = waves * (ty + 0.7) * (xc + 3) * (1.0 + 0.02 * (tymax - ty)) * march;
       if (cost < best) {
         best = cost;
         pl.ok = true; pl.ty = ty; pl.stages = S; pl.xc = xc; pl.tiles = tiles;
@@ -252,14 +256,9 @@ bool encode_field_map(monc_adv_t h, CUtensorMap *m, const void *base, int box_z,
   const cuuint32_t estr[3] = {1u, 1u, 1u};
   const CUtensorMapDataType dt =
       sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-  static const int promo = []() { const char *e = getenv("MONC_ADV_L2PROMO"); return e ? atoi(e) : 3; }();
-  const CUtensorMapL2promotion pr = promo == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
-                                  : promo == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
-                                  : promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
-                                               : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
   return enc(m, dt, 3, const_cast<void *>(base), gdim, gstr, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-             pr, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // geometry of tma_scalars: ty columns x zw z-chunks (32 vectors each) x ss
@@ -323,7 +322,11 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
             const int xc = (nplanes + nch - 1) / nch;
             const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
             const long waves = (blocks + h->sm_count - 1) / h->sm_count;
-            const double cost = (double)waves * (xc + 4) * t_step;  // +2 halo planes, ~2 steps of start-up latency
+            // +2 halo planes, ~2 steps of start-up latency; on a long march the y/z
+            // neighbours drift apart and their halo re-reads miss L2 (config 2: DRAM
+            // reads 8.9 GB at xc = 512 against 7.7 GB at xc = 64, 11 % slower)
+            const double march = 1.0 + 0.2 * std::min(xc, 512) / 512.0;
+            const double cost = (double)waves * (xc + 4) * t_step * march;
             if (cost < best) {
               best = cost;
               pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
