@@ -228,6 +228,8 @@ def run_ours(args):
         L.set_variant(args.variant)
     if args.no_pdl:
         L.set_pdl(False)
+    if args.form != "flux":
+        L.set_form(args.form)
     tdt = L.torch_dtype
     # weak scaling: every rank advects its own subdomain of the config's size
     # ("replicas only" until the halo-exchange row of SURVEY.md 8(f) is built);
@@ -380,7 +382,7 @@ def run_ours(args):
     tsuf = "double" if cfg.dtype == "f64" else "float"
     achieved = kb / (kms * 1e-3) / 1e9
     traffic, traffic_src = args.traffic, "--traffic"
-    tuned = any((args.xchunk, args.group, args.stages, args.tile_y, args.warps, args.split))
+    tuned = any((args.xchunk, args.group, args.stages, args.tile_y, args.warps, args.split)) or args.form != "flux"
     if traffic is None and not tuned:
         traffic, traffic_src = NCU_TRAFFIC.get((args.workload, f"{fam}_{kern}"), (None, None))
     roofline = {"bound": "hbm", "kernel": f"{fam}_{kern}<{tsuf}>", "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -410,7 +412,7 @@ def run_ours(args):
                                    else ("replicas only" if world > 1 else "1 GPU")),
                    "variant": args.variant or "auto", "xchunk": args.xchunk, "group": args.group,
                    "stages": args.stages, "tile_y": args.tile_y, "warps": args.warps,
-                   "split": args.split, "pdl": not args.no_pdl, "launch_plan": plan},
+                   "split": args.split, "pdl": not args.no_pdl, "form": args.form, "launch_plan": plan},
         "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
@@ -533,9 +535,22 @@ def cpu_baseline(cfg, args):
         dt = time.perf_counter() - t0
         if dt > args.cpu_seconds:
             break
+    # the same loops threaded over (i, j) on every host core
+    nthr = oracle.max_threads()
+    reps_all, t1 = 0, time.perf_counter()
+    while True:
+        P.momentum(H[0], H[1], H[2], nthreads=nthr, out=outs)
+        for q in H[3:]:
+            P.scalar(H[0], H[1], H[2], q, nthreads=nthr, out=sq)
+        reps_all += 1
+        dt_all = time.perf_counter() - t1
+        if dt_all > args.cpu_seconds / 3:
+            break
     return {"value": sub.points * reps / dt / 1e9, "unit": "Gpts/s", "cores": 1, "kind": "oracle",
             "sample": f"{reps} oracle passes (fp64, 1 thread) over the first {sub.nx} of {cfg.nx}"
                       f" x-planes of {args.workload}, {len(names)} fields, {dt:.1f} s",
+            "all_cores": {"value": sub.points * reps_all / dt_all / 1e9, "unit": "Gpts/s", "cores": nthr,
+                          "sample": f"{reps_all} passes of the same sample, {dt_all:.1f} s"},
             "host_cores_available": len(os.sched_getaffinity(0))}
 
 
@@ -557,6 +572,8 @@ def main():
     ap.add_argument("--event-every", type=int, default=10,
                     help="momentum-only workloads: launches between two timing events")
     ap.add_argument("--no-pdl", action="store_true", help="plain stream order between kernels")
+    ap.add_argument("--form", default="flux", choices=["flux", "pw_skew"],
+                    help="flux form (default, BASELINE.json) or the Piacsek-Williams skew form (DESIGN.md R4)")
     ap.add_argument("--ref-planes", type=int, default=64)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--halo-exchange", action="store_true",
