@@ -110,6 +110,23 @@ int pick_xchunk(monc_adv_t h, int nplanes, int blocks_per_plane, int resident_pe
   return std::min(xc, nplanes);
 }
 
+// How many block-times a launch of `blocks` equal blocks (one resident per SM)
+// takes.  Measured on B200: a GPC sustains about 16 SMs' worth
+// of these streaming kernels.  Up to 8 x 16 = 128 blocks run at the full per-SM
+// rate; a single static wave of 129..148 blocks is as slow as its fullest GPC
+// (20 SMs on 16 SMs' worth of bandwidth: 1.27 x at 148 blocks); many waves are
+// balanced dynamically (about 1.12 block-times per 148 blocks), and a partial
+// last wave costs a whole block-time again.
+double launch_rounds(long blocks, int sm_count) {
+  const long full_rate = std::max(1L, (long)sm_count * 128 / 148);
+  auto one_wave = [&](long b) {
+    return b <= full_rate ? 1.0 : 1.0 + 0.27 * (double)(b - full_rate) / (double)(sm_count - full_rate);
+  };
+  if (blocks <= sm_count) return one_wave(blocks);
+  const long full = blocks / sm_count, rem = blocks % sm_count;
+  return 1.12 * full + (rem ? one_wave(rem) : 0.0);
+}
+
 // geometry of the TMA-staged kernels: TY columns per block, ring depth S
 struct TmaPlan {
   bool ok = false;
@@ -141,15 +158,11 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
     for (int nch = nch_lo; nch <= nch_hi; ++nch) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
-      // few blocks per SM run in lock-step waves; many are balanced dynamically
-      const double waves = blocks <= 6L * h->sm_count
-                               ? (double)((blocks + h->sm_count - 1) / h->sm_count)
-                               : (double)blocks / h->sm_count;
-      // time ~ waves * (columns per block + the L2/shared-memory cost of its two halo
-      // columns) * (planes per block + ramp-up planes) * (long marches: SMs get unequal
-      // shares of HBM and y neighbours drift apart, measured +11 % from 32 to 64 planes)
-      const double march = 1.0 + 0.12 * std::min(xc, 64) / 32.0;
-      const double cost = waves * (ty + 0.7) * (xc + 3) * (1.0 + 0.02 * (tymax - ty)) * march;
+      // time ~ block-times of the launch * (columns per block + the L2/shared-memory
+      // cost of its two halo columns) * (planes per block + its two halo planes)
+      const double rounds = launch_rounds(blocks, h->sm_count);
+      const double march = 1.0 + 0.1 * std::min(xc, 256) / 256.0;  // y neighbours drift apart
+      const double cost = rounds * (ty + 0.7) * (xc + 2) * (1.0 + 0.02 * (tymax - ty)) * march;
       if (cost < best) {
         best = cost;
         pl.ok = true; pl.ty = ty; pl.stages = S; pl.xc = xc; pl.tiles = tiles;
@@ -321,12 +334,12 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
           for (int nch = nch_lo; nch <= nch_hi; ++nch) {
             const int xc = (nplanes + nch - 1) / nch;
             const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
-            const long waves = (blocks + h->sm_count - 1) / h->sm_count;
+            const double waves = launch_rounds(blocks, h->sm_count);
             // +2 halo planes, ~2 steps of start-up latency; on a long march the y/z
             // neighbours drift apart and their halo re-reads miss L2 (config 2: DRAM
             // reads 8.9 GB at xc = 512 against 7.7 GB at xc = 64, 11 % slower)
             const double march = 1.0 + 0.2 * std::min(xc, 512) / 512.0;
-            const double cost = (double)waves * (xc + 4) * t_step * march;
+            const double cost = waves * (xc + (waves <= 1.3 ? 4 : 2)) * t_step * march;
             if (cost < best) {
               best = cost;
               pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
