@@ -148,9 +148,9 @@ def workload_cfg(name):
 # kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
 # by (workload, kernel family); valid for the library's default launch plan only.
 NCU_TRAFFIC = {
-    ("config1", "tma_momentum"): (365.3e6, "profiles/r01_config1_tma_momentum_f64.md"),
-    ("config2", "tma_scalars"): (13009.9e6, "profiles/r01_config2_tma_scalars_f64.md"),
-    ("config3", "tma_scalars"): (6253.7e6, "profiles/r01_config3_tma_f32.md"),
+    ("config1", "tma_momentum"): (358.1e6, "profiles/r01_config1_tma_momentum_f64.md"),
+    ("config2", "tma_scalars"): (12970.8e6, "profiles/r01_config2_tma_scalars_f64.md"),
+    ("config3", "tma_scalars"): (6222.6e6, "profiles/r01_config3_tma_f32.md"),
 }
 
 
