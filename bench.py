@@ -332,7 +332,7 @@ def run_ours(args):
     for t_, a in zip(hin, H):
         t_.copy_(torch.from_numpy(a))
     hout = [torch.zeros(L.shape, dtype=tdt, pin_memory=True) for _ in names]
-    L.set_chunks(8)
+    L.set_chunks(args.chunks)
 
     def e2e_step():
         L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
@@ -417,7 +417,7 @@ def run_ours(args):
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
                 "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
-                "phase_ms": phase, "chunks": 8, "serial_phase_ms": serial,
+                "phase_ms": phase, "chunks": args.chunks, "serial_phase_ms": serial,
                 "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / phase["total"],
                 "timing": "host wall clock around step_async + step_wait, pinned host buffers"},
         "gpu_launches": launches, "clocks": clocks,
@@ -579,7 +579,7 @@ def main():
     ap.add_argument("--halo-exchange", action="store_true",
                     help="N ranks advect x-slabs of ONE periodic domain of N*nx planes and swap halos over NCCL every step"
                          " (default: independent replicas, no data-path collective)")
-    ap.add_argument("--chunks", type=int, default=8, help="config4: x-slab chunks per step")
+    ap.add_argument("--chunks", type=int, default=8, help="x-slab chunks per hybrid step (BASELINE.json config 4: 8)")
     ap.add_argument("--no-perturb", action="store_true", help="config4: keep the fields fixed between steps")
     ap.add_argument("--traffic", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel, if known")
