@@ -155,8 +155,10 @@ int monc_adv_set_chunks(monc_adv_t h, int nchunks);
  * work serialised on one stream (H2D all, kernels, D2H all) -- the baseline
  * for the overlap ratio. */
 int monc_adv_set_overlap(monc_adv_t h, int on);
-/* MONC_ADV_FORM_FLUX (default) or MONC_ADV_FORM_PW_SKEW (SURVEY.md 8(f)
- * NEXT-1: centre value dropped from every advected-quantity parenthesis). */
+/* MONC_ADV_FORM_FLUX (default) or MONC_ADV_FORM_PW_SKEW (PAPER.md:97 names the
+ * Piacsek-Williams scheme; the centre value is
+ * dropped from every advected-quantity parenthesis).  Both forms run on the
+ * generic kernels and on the TMA kernels (variants 1 and 3). */
 int monc_adv_set_form(monc_adv_t h, int form);
 /* 0 (default): tendencies overwritten.  1: added into the output buffers. */
 int monc_adv_set_accumulate(monc_adv_t h, int on);
@@ -168,7 +170,7 @@ int monc_adv_set_pdl(monc_adv_t h, int on);
 /* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
  * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
  * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need
- * nz % (16/sizeof(dtype)) == 0 and the flux form. */
+ * nz % (16/sizeof(dtype)) == 0; 2 also needs the flux form. */
 int monc_adv_set_variant(monc_adv_t h, int variant);
 /* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
  * that makes sense.

@@ -154,7 +154,7 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
     if (S < 3) continue;
     const int tiles = (h->ny + ty - 1) / ty;
     const int nch_lo = nch_fixed ? nch_fixed : 1;
-    const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 8);
+    const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 4);
     for (int nch = nch_lo; nch <= nch_hi; ++nch) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
