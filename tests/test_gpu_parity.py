@@ -351,3 +351,48 @@ def test_user_supplied_tz_arrays_and_stream():
         gc.check(cfg, o, w_, n)
     assert L.launch_count() == 1
     L.close()
+
+
+# ---------------------------------------------------------------------------
+# guard bands: nothing outside the caller's arrays is read into a result or written
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
+@pytest.mark.parametrize("form", ["flux", "pw_skew"])
+def test_guard_bands(dtype, variant, form):
+    """Every field sits inside a larger allocation whose guard regions hold NaN
+    (inputs) or a sentinel (outputs), with the tightest halo (1).  A read past
+    an array that reaches a result shows up as NaN (0 * NaN included); a write
+    past an output array changes its guard."""
+    if variant == "march" and form == "pw_skew":
+        pytest.skip("march kernels are flux-form only")
+    cfg = gc.custom_cfg(9, 10, 72, halo=1, nq=3, dtype=dtype, cid=307)
+    P, L = gc.make_pair(cfg)
+    L.set_variant(variant)
+    L.set_form(form)
+    L.set_tuning(xchunk=4)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    n = int(np.prod(L.shape))
+    G = 4096  # guard elements on each side (keeps 16-byte alignment)
+
+    def embed(a, fill):
+        buf = torch.full((n + 2 * G,), fill, device="cuda", dtype=L.torch_dtype)
+        view = buf[G:G + n].view(L.shape)
+        if a is not None:
+            view.copy_(torch.from_numpy(a).to(L.torch_dtype))
+        return buf, view
+
+    ins = [embed(a, float("nan")) for a in H]
+    outs = [embed(None, gc.SENTINEL) for _ in range(3 + cfg.nq)]
+    L.momentum(ins[0][1], ins[1][1], ins[2][1], outs[0][1], outs[1][1], outs[2][1])
+    L.scalars([b[1] for b in ins[3:]], [b[1] for b in outs[3:]])
+    torch.cuda.synchronize()
+    skew = form == "pw_skew"
+    want = list(P.momentum(H[0], H[1], H[2], skew=skew)) + [P.scalar(H[0], H[1], H[2], q, skew=skew) for q in H[3:]]
+    for (buf, view), w_, nm in zip(outs, want, ["su", "sv", "sw"] + names[3:]):
+        gc.check(cfg, view, w_, nm)
+        gc.check_halo_untouched(cfg, view, nm)
+        g = buf.cpu().numpy()
+        assert np.all(g[:G] == gc.SENTINEL) and np.all(g[G + n:] == gc.SENTINEL), f"{nm}: guard written"
+    L.close()
