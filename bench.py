@@ -334,19 +334,25 @@ def run_ours(args):
     hout = [torch.zeros(L.shape, dtype=tdt, pin_memory=True) for _ in names]
     L.set_chunks(args.chunks)
 
+    enqueue_s = [0.0]
+
     def e2e_step():
+        te = time.perf_counter()
         L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+        enqueue_s[0] += time.perf_counter() - te  # the host is free from here
         L.step_wait()
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     for _ in range(2):
         e2e_step()
     barrier()
+    enqueue_s[0] = 0.0
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         e2e_step()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    enqueue_ms = enqueue_s[0] / e2e_steps * 1e3
     phase = L.step_times_ms()
     # the same step with copies and kernels serialised on one stream: its phases are
     # the "alone" times of the overlap ratio
@@ -416,6 +422,7 @@ def run_ours(args):
         "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
         "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
                 "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
+                "host_enqueue_ms_per_step": enqueue_ms,
                 "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
                 "phase_ms": phase, "chunks": args.chunks, "serial_phase_ms": serial,
                 "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / phase["total"],
