@@ -396,7 +396,10 @@ def run_ours(args):
                 "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
                 "best_launch_ms": best["mom" if kern == "momentum" else "sca"],
                 "launches_per_event": grp if kern == "momentum" else 1,
-                "frac_of_nominal_8TBs": achieved / 8000.0}
+                "frac_of_nominal_8TBs": achieved / 8000.0,
+                # BASELINE.json's "achieved HBM GB/s from ncu": the profiled DRAM bytes of
+                # one launch over this run's measured launch time
+                "ncu_dram_GBs": (traffic / (kms * 1e-3) / 1e9) if traffic else None}
     kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
     if args.halo_exchange:
         kernels["halo_swap_ms"] = swap_avg
