@@ -82,6 +82,29 @@ def test_step_async_small(nchunks, overlap, dtype):
     L.close()
 
 
+def test_step_async_pw_skew():
+    # the hybrid step in the PW-skew form (NEXT-1): x-slab launches of the TMA kernels
+    cfg = gc.custom_cfg(24, 17, 128, nq=4, cid=403)
+    P, L = gc.make_pair(cfg)
+    L.set_form("pw_skew")
+    L.set_chunks(5)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    names = synth.field_names(cfg)
+    Q = [synth.field(cfg, n) for n in names]
+    hin = [pinned(a, L) for a in (U, V, W)]
+    hq = [pinned(a, L) for a in Q]
+    hout, hsq = pinned_out(L, 3), pinned_out(L, 4)
+    L.step_async(*hin, hq, *hout, hsq)
+    L.step_wait()
+    assert "tma_momentum" in L.describe_plan() and "tma_scalars" in L.describe_plan()
+    for o, w_, n in zip(hout, P.momentum(U, V, W, skew=True), ("su", "sv", "sw")):
+        gc.check(cfg, o, w_, n)
+        gc.check_halo_untouched(cfg, o, n)
+    for o, q, n in zip(hsq, Q, names):
+        gc.check(cfg, o, P.scalar(U, V, W, q, skew=True), n)
+    L.close()
+
+
 def test_step_async_after_user_stream_work():
     cfg = gc.custom_cfg(16, 8, 32, cid=401)
     P, L = gc.make_pair(cfg)
