@@ -110,6 +110,20 @@ int monc_adv_bind_wind(monc_adv_t h, const void *u, const void *v, const void *w
 int monc_adv_scalars(monc_adv_t h, const void *const *q, void *const *sq, int nq,
                      void *cuda_stream);
 
+/* The whole step from device arrays in one call (the lower bound
+ * of 24 + 24 + 16 nq bytes per point is reached only if u, v, w are read once
+ * for momentum AND scalars; "u, v and w ... shared between kernels").
+ * Same results (same arithmetic; only the compiler's FMA contraction may differ)
+ * as monc_adv_momentum(u, v, w, su, sv, sw) followed by monc_adv_scalars(q, sq,
+ * nq); binds (u, v, w) as the wind.  With 1 <= nq <=
+ * 10 and a TMA plan that fits, ONE launch does both (the momentum role rides in
+ * the scalar kernel's thread blocks and reads the same staged wind tiles);
+ * otherwise the two launches are made.  Arguments, layout, ownership and errors
+ * as for the two calls; all outputs must be distinct and alias no input. */
+int monc_adv_tendencies(monc_adv_t h, const void *u, const void *v, const void *w, void *su,
+                        void *sv, void *sw, const void *const *q, void *const *sq, int nq,
+                        void *cuda_stream);
+
 /*
  * The paper's hybrid pattern:
  * fields live in PINNED HOST memory; the call enqueues, per x-slab chunk, the
@@ -167,6 +181,9 @@ int monc_adv_set_accumulate(monc_adv_t h, int on);
  * predecessor in the stream (it waits for the predecessor's completion before
  * touching any field: results are unchanged).  0: plain stream order. */
 int monc_adv_set_pdl(monc_adv_t h, int on);
+/* 1 (default): monc_adv_tendencies and monc_adv_step_async use the fused
+ * momentum + scalars launch where it fits.  0: always two launches. */
+int monc_adv_set_fuse(monc_adv_t h, int on);
 /* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
  * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
  * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need

@@ -26,7 +26,7 @@ MAX_SCALARS = 64
 # every symbol include/monc_adv.h declares (tests check the .so exports them all)
 SYMBOLS = [
     "monc_adv_create", "monc_adv_destroy", "monc_adv_momentum", "monc_adv_bind_wind",
-    "monc_adv_scalars", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
+    "monc_adv_scalars", "monc_adv_tendencies", "monc_adv_set_fuse", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
     "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range",
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
@@ -64,6 +64,8 @@ def load():
     lib.monc_adv_bind_wind.restype = ci
     lib.monc_adv_scalars.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), ci, vp]
     lib.monc_adv_scalars.restype = ci
+    lib.monc_adv_tendencies.argtypes = [vp] * 7 + [C.POINTER(vp), C.POINTER(vp), ci, vp]
+    lib.monc_adv_tendencies.restype = ci
     lib.monc_adv_step_async.argtypes = [vp, vp, vp, vp, C.POINTER(vp), ci, vp, vp, vp, C.POINTER(vp), vp]
     lib.monc_adv_step_async.restype = ci
     for name in ("monc_adv_step_inputs_consumed", "monc_adv_step_wait"):
@@ -76,7 +78,8 @@ def load():
     lib.monc_adv_step_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
-                 "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant"):
+                 "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
+                 "monc_adv_set_fuse"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -189,6 +192,15 @@ class MoncAdv:
         sp = self._table([self._dev(t, f"sq[{n}]") for n, t in enumerate(sq)])
         self._check(self._lib.monc_adv_scalars(self._h, qp, sp, len(q), _stream_ptr(stream)))
 
+    def tendencies(self, u, v, w, su, sv, sw, q, sq, stream=None):
+        if len(q) != len(sq):
+            raise MoncAdvError(EINVAL, "tendencies: len(q) != len(sq)")
+        args = [self._dev(t, n) for t, n in zip((u, v, w, su, sv, sw), ("u", "v", "w", "su", "sv", "sw"))]
+        qp = self._table([self._dev(t, f"q[{n}]") for n, t in enumerate(q)])
+        sp = self._table([self._dev(t, f"sq[{n}]") for n, t in enumerate(sq)])
+        self._wind_keepalive = (u, v, w)
+        self._check(self._lib.monc_adv_tendencies(self._h, *args, qp, sp, len(q), _stream_ptr(stream)))
+
     def step_async(self, hu, hv, hw, hq, hsu, hsv, hsw, hsq, stream=None):
         hq, hsq = list(hq or []), list(hsq or [])
         if len(hq) != len(hsq):
@@ -239,6 +251,9 @@ class MoncAdv:
 
     def set_pdl(self, on):
         self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
+
+    def set_fuse(self, on):
+        self._check(self._lib.monc_adv_set_fuse(self._h, int(bool(on))))
 
     def set_variant(self, variant):
         variant = {"auto": 0, "generic": 1, "march": 2, "tma": 3}.get(variant, variant)

@@ -33,7 +33,7 @@ struct monc_adv_s {
   void *d_tz[4] = {nullptr, nullptr, nullptr, nullptr};  // tzc1, tzc2, tzd1, tzd2 (dtype)
   std::vector<double> tz_host[4];                        // as stored on the device
   const void *wind[3] = {nullptr, nullptr, nullptr};
-  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1;
+  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1, fuse = 1;
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
@@ -285,7 +285,7 @@ struct TmaScalarPlan {
 };
 
 template <typename T>
-TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
+TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = false) {
   TmaScalarPlan pl;
   constexpr int NK = VecOf<T>::NK;
   if (h->nz % NK != 0 || !tensor_map_encoder()) return pl;
@@ -304,6 +304,7 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
     if (h->group > 0 && gb != std::min(h->group, std::min(n, 10))) continue;
     if (h->group == 0 && gb != std::min(n, 5) && gb != std::min(n, 10)) continue;
     const int ngroups = (n + gb - 1) / gb;
+    if (mom && ngroups != 1) continue;  // the momentum role runs once: one group holds every scalar
     for (int ss = 1; ss <= std::min(gb, 4); ++ss) {
       if (h->split > 0 && ss != std::min(h->split, std::min(gb, 4))) continue;
       const int gw = (gb + ss - 1) / ss;
@@ -312,7 +313,7 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
         if (h->warps > 0 && zw != std::min(h->warps, zwmax)) continue;
         const int ZB = zw * 32 * NK, RS = ZB + 2 * NK;
         const int nzt = (h->nz + ZB - 1) / ZB;
-        const int tymax = std::min(h->ny, kScalarConsumerWarps / (zw * ss));
+        const int tymax = std::min(h->ny, kScalarConsumerWarps / (zw * (ss + (mom ? 1 : 0))));
         if (tymax < 1) continue;
         for (int ty = tymax; ty >= 1; --ty) {
           if (h->tile_y > 0 && ty != std::min(h->tile_y, tymax)) continue;
@@ -320,13 +321,13 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
           const size_t stage = (size_t)(3 + gb) * field;
           int S = (int)std::min<size_t>(8, budget / (stage + 16));
           if (h->stages > 0) S = std::min(S, h->stages);
-          if (S < 2) continue;
+          if (S < (mom ? 3 : 2)) continue;
           const int tiles = ((h->ny + ty - 1) / ty) * nzt * ngroups;
           // the groups after the first re-read the wind; about half of that hits L2
           const double wind = 3.0 * (1.0 + 0.5 * (ngroups - 1)) / ngroups;
-          const double dram_b = ((wind + gb) + gb) * ty * ZB * sizeof(T);
+          const double dram_b = ((wind + gb) + gb + (mom ? 3 : 0)) * ty * ZB * sizeof(T);
           const double t_mem = dram_b / (sm_gbs * 1e3);                            // us
-          const double t_warp = 0.15 + 0.25 * gw;                                    // us
+          const double t_warp = std::max(0.15 + 0.25 * gw, mom ? 1.2 : 0.0);         // us; momentum ~ 4 scalars
           const double shallow = S >= 3 ? 1.0 : 1.15;
           const double t_step = std::max(t_mem, t_warp) * shallow + 0.05;
           const int nch_lo = nch_fixed ? nch_fixed : 1;
@@ -356,39 +357,50 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n) {
   return pl;
 }
 
-template <typename T, int GW, bool ACC, bool SKEW>
-int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
-                         const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC, SKEW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
+int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
+                         const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC, SKEW, MOM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                          (int)pl.smem));
   dim3 grid(pl.tiles, pl.nchunks);
-  const int threads = (pl.ty * pl.zw * pl.ss + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW>, grid, threads, pl.smem, st, p, maps, outs, nq,
+  const int threads = (pl.ty * pl.zw * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
                 (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
 }
 
-template <typename T, int GW>
-int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps,
-                       const SqPtrs<T> &outs, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+template <typename T, int GW, bool MOM>
+int launch_tma_scalars_m(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
+                         const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
   const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
   if (h->accumulate)
-    return skew ? launch_tma_scalars_k<T, GW, true, true>(h, p, maps, outs, nq, pl, st)
-                : launch_tma_scalars_k<T, GW, true, false>(h, p, maps, outs, nq, pl, st);
-  return skew ? launch_tma_scalars_k<T, GW, false, true>(h, p, maps, outs, nq, pl, st)
-              : launch_tma_scalars_k<T, GW, false, false>(h, p, maps, outs, nq, pl, st);
+    return skew ? launch_tma_scalars_k<T, GW, true, true, MOM>(h, p, maps, outs, mo, nq, pl, st)
+                : launch_tma_scalars_k<T, GW, true, false, MOM>(h, p, maps, outs, mo, nq, pl, st);
+  return skew ? launch_tma_scalars_k<T, GW, false, true, MOM>(h, p, maps, outs, mo, nq, pl, st)
+              : launch_tma_scalars_k<T, GW, false, false, MOM>(h, p, maps, outs, mo, nq, pl, st);
+}
+
+template <typename T, int GW>
+int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
+                       const MomPtrs<T> *mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
+  if (mo) return launch_tma_scalars_m<T, GW, true>(h, p, maps, outs, *mo, nq, pl, st);
+  return launch_tma_scalars_m<T, GW, false>(h, p, maps, outs, MomPtrs<T>{nullptr, nullptr, nullptr}, nq, pl, st);
 }
 
 // One launch of tma_scalars per kMaxScalarsPerLaunch scalars.  *done = false
 // with MONC_ADV_OK means "does not fit, nothing launched": the caller falls back.
+// mo != nullptr: the fused launch (momentum role included); it needs every
+// scalar in ONE group of one launch, otherwise nothing is launched.
 template <typename T>
 int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T *w,
                     const void *const *q, void *const *sq, int nq, int ia, int ib,
-                    cudaStream_t st, bool *done) {
+                    cudaStream_t st, bool *done, const MomPtrs<T> *mo = nullptr) {
   *done = false;
   constexpr int NK = VecOf<T>::NK;
+  if (mo && nq > 10) return MONC_ADV_OK;
   for (int base = 0; base < nq; base += kMaxScalarsPerLaunch) {
     const int n = std::min(kMaxScalarsPerLaunch, nq - base);
-    const TmaScalarPlan pl = plan_tma_scalars<T>(h, ib - ia, n);
+    const TmaScalarPlan pl = plan_tma_scalars<T>(h, ib - ia, n, mo != nullptr);
     if (!pl.ok) {
       if (base == 0) return MONC_ADV_OK;
       return fail(h, MONC_ADV_ECUDA, "scalars: TMA plan failed after a partial launch");
@@ -408,20 +420,22 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
     p.xc = pl.xc;
     int rc = MONC_ADV_OK;
     switch (pl.gw) {
-      case 1: rc = launch_tma_scalars<T, 1>(h, p, maps, outs, n, pl, st); break;
-      case 2: rc = launch_tma_scalars<T, 2>(h, p, maps, outs, n, pl, st); break;
-      case 3: rc = launch_tma_scalars<T, 3>(h, p, maps, outs, n, pl, st); break;
-      case 4: rc = launch_tma_scalars<T, 4>(h, p, maps, outs, n, pl, st); break;
-      default: rc = launch_tma_scalars<T, 5>(h, p, maps, outs, n, pl, st); break;
+      case 1: rc = launch_tma_scalars<T, 1>(h, p, maps, outs, mo, n, pl, st); break;
+      case 2: rc = launch_tma_scalars<T, 2>(h, p, maps, outs, mo, n, pl, st); break;
+      case 3: rc = launch_tma_scalars<T, 3>(h, p, maps, outs, mo, n, pl, st); break;
+      case 4: rc = launch_tma_scalars<T, 4>(h, p, maps, outs, mo, n, pl, st); break;
+      default: rc = launch_tma_scalars<T, 5>(h, p, maps, outs, mo, n, pl, st); break;
     }
     if (rc != MONC_ADV_OK) return rc;
     CU(cudaGetLastError());
     h->launches++;
     char b[200];
-    snprintf(b, sizeof b, "tma_scalars group=%d per_warp=%d split=%d ty=%d zw=%d stages=%d xc=%d grid=%dx%d "
-             "threads=%d smem=%zu", pl.gb, pl.gw, pl.ss, pl.ty, pl.zw, pl.stages, pl.xc, pl.tiles,
-             pl.nchunks, (pl.ty * pl.zw * pl.ss + 1) * 32, pl.smem);
+    snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d zw=%d stages=%d xc=%d grid=%dx%d "
+             "threads=%d smem=%zu", mo ? "tma_fused(momentum+scalars)" : "tma_scalars", pl.gb, pl.gw, pl.ss,
+             pl.ty, pl.zw, pl.stages, pl.xc, pl.tiles, pl.nchunks,
+             (pl.ty * pl.zw * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
     h->plan_sca = b;
+    if (mo) h->plan_mom.clear();
   }
   *done = true;
   return MONC_ADV_OK;
@@ -476,6 +490,23 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
   CU(cudaGetLastError());
   h->launches++;
   return MONC_ADV_OK;
+}
+
+// whole step from device arrays: one fused launch when the plan allows it, else
+// the momentum launch followed by the scalars launch
+template <typename T>
+int launch_tendencies(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
+                      const void *const *q, void *const *sq, int nq, int ia, int ib, cudaStream_t st) {
+  if (nq > 0 && h->fuse && (h->variant == 3 || h->variant == 0)) {
+    KParams<T> p = make_params<T>(h, ia, ib);
+    const MomPtrs<T> mo{su, sv, sw};
+    bool done = false;
+    const int rc = run_tma_scalars<T>(h, p, u, v, w, q, sq, nq, ia, ib, st, &done, &mo);
+    if (rc != MONC_ADV_OK || done) return rc;
+  }
+  const int rc = launch_momentum<T>(h, u, v, w, su, sv, sw, ia, ib, st);
+  if (rc != MONC_ADV_OK || nq == 0) return rc;
+  return launch_scalars<T>(h, u, v, w, q, sq, nq, ia, ib, st);
 }
 
 int check_handle(monc_adv_t h) {
@@ -585,9 +616,9 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
     CU(cudaEventRecord(h->ev_kb[c], sk));
     int rc = MONC_ADV_OK;
     if (mom)
-      rc = launch_momentum<T>(h, du, dv, dw, (T *)h->d_out[0], (T *)h->d_out[1],
-                              (T *)h->d_out[2], ia, ib, sk);
-    if (rc == MONC_ADV_OK && nq > 0)
+      rc = launch_tendencies<T>(h, du, dv, dw, (T *)h->d_out[0], (T *)h->d_out[1], (T *)h->d_out[2],
+                                dq.data(), dsq.data(), nq, ia, ib, sk);
+    else if (nq > 0)
       rc = launch_scalars<T>(h, du, dv, dw, dq.data(), dsq.data(), nq, ia, ib, sk);
     if (rc != MONC_ADV_OK) return rc;
     CU(cudaEventRecord(h->ev_ke[c], sk));
@@ -774,6 +805,44 @@ int monc_adv_scalars(monc_adv_t h, const void *const *q, void *const *sq, int nq
                                   (const double *)h->wind[2], q, sq, nq, h->h, h->h + h->nx, st);
   return launch_scalars<float>(h, (const float *)h->wind[0], (const float *)h->wind[1],
                                (const float *)h->wind[2], q, sq, nq, h->h, h->h + h->nx, st);
+}
+
+int monc_adv_tendencies(monc_adv_t h, const void *u, const void *v, const void *w, void *su,
+                        void *sv, void *sw, const void *const *q, void *const *sq, int nq,
+                        void *cuda_stream) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!u || !v || !w || !su || !sv || !sw) return fail(h, MONC_ADV_EINVAL, "tendencies: NULL pointer");
+  if (nq < 0 || nq > MONC_ADV_MAX_SCALARS) return fail(h, MONC_ADV_EINVAL, "tendencies: nq out of range");
+  if (nq > 0 && (!q || !sq)) return fail(h, MONC_ADV_EINVAL, "tendencies: NULL pointer table");
+  std::vector<const void *> ins = {u, v, w}, outs = {su, sv, sw};
+  for (int n = 0; n < nq; ++n) {
+    if (!q[n] || !sq[n]) return fail(h, MONC_ADV_EINVAL, "tendencies: NULL field pointer");
+    ins.push_back(q[n]);
+    outs.push_back(sq[n]);
+  }
+  for (const void *p : ins)
+    if (!aligned16(p)) return fail(h, MONC_ADV_EINVAL, "tendencies: pointers must be 16-byte aligned");
+  for (size_t b = 0; b < outs.size(); ++b) {
+    if (!aligned16(outs[b])) return fail(h, MONC_ADV_EINVAL, "tendencies: pointers must be 16-byte aligned");
+    for (const void *a : ins)
+      if (a == outs[b]) return fail(h, MONC_ADV_EINVAL, "tendencies: inputs and outputs must not alias");
+    for (size_t c = 0; c < b; ++c)
+      if (outs[c] == outs[b]) return fail(h, MONC_ADV_EINVAL, "tendencies: outputs must be distinct");
+  }
+  h->wind[0] = u; h->wind[1] = v; h->wind[2] = w;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->dtype == MONC_ADV_F64)
+    return launch_tendencies<double>(h, (const double *)u, (const double *)v, (const double *)w, (double *)su,
+                                     (double *)sv, (double *)sw, q, sq, nq, h->h, h->h + h->nx, st);
+  return launch_tendencies<float>(h, (const float *)u, (const float *)v, (const float *)w, (float *)su,
+                                  (float *)sv, (float *)sw, q, sq, nq, h->h, h->h + h->nx, st);
+}
+
+int monc_adv_set_fuse(monc_adv_t h, int on) {
+  if (!h) return MONC_ADV_EINVAL;
+  h->fuse = on ? 1 : 0;
+  return MONC_ADV_OK;
 }
 
 int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void *hw,

@@ -145,6 +145,107 @@ struct XFlux {
   Vec<T> xx, xy, xz;
 };
 
+// the values one level below a warp's first level (lane 0 of the upper z chunks)
+template <typename T>
+struct BelowEdge {
+  T ub, vb, wb, web, wnb;  // u, v, w of the centre plane; w of the east plane and of the north column
+};
+
+// ---------------------------------------------------------------------------
+// One x step of the fused momentum update for a thread's NK levels (SURVEY.md
+// 8(c).2 blocks su/sv/sw): centre plane RC, east plane RE, the centre plane's
+// south/north/upper neighbours, the west-face terms FW carried from the
+// previous step.  Returns the tendencies of the centre plane and, in FE, the
+// east-face terms the next step needs as its west.
+// ---------------------------------------------------------------------------
+template <typename T, bool SKEW>
+__device__ __forceinline__ void momentum_faces(
+    const PlaneRegs<T> &RC, const PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE,
+    const Vec<T> &uS, const Vec<T> &uN, const Vec<T> &vN, const Vec<T> &wS, const Vec<T> &wN,
+    const Vec<T> &uCu, const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const bool bot_edge,
+    const BelowEdge<T> &be, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1, const Vec<T> &d2,
+    const T cx, const T cy, const int lane, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
+  constexpr int NK = VecOf<T>::NK;
+  T b_xz = T(0), b_yz = T(0), b_zz = T(0);
+  if (bot_edge) {
+    const T ub = be.ub, vb = be.vb, wb = be.wb, web = be.web, wnb = be.wnb;
+    if (SKEW) {
+      b_xz = ub * (wb + web);
+      b_yz = vb * (wb + wnb);
+      b_zz = wb * (wb + RC.w.v[0]);
+    } else {
+      b_xz = (ub + RC.u.v[0]) * (wb + web);
+      b_yz = (vb + RC.v.v[0]) * (wb + wnb);
+      b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
+    }
+  }
+  if (SKEW) {
+    // Piacsek-Williams skew form (R4): the advected parenthesis holds the
+    // neighbour's value only, so a face carries two products, A*phi_far for the
+    // point on this side and A*phi_near for the point across the face (handed on
+    // through FE in x, by shuffle in z), with the advecting sums A shared.
+    Vec<T> su_t, sv_t, sw_t, pu_t, pv_t, pw_t, ry, rv, rwy;
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      const T axu = RC.u.v[e] + RE.u.v[e];     // advects u through the east face
+      const T axv = RC.u.v[e] + uN.v[e];       // advects v through the east face
+      const T axw = RC.u.v[e] + uCu.v[e];      // advects w through the east face
+      const T ayu_n = RC.v.v[e] + RE.v.v[e], ayu_s = RC.vs.v[e] + RE.vs.v[e];
+      const T ayv_n = RC.v.v[e] + vN.v[e], ayv_s = RC.vs.v[e] + RC.v.v[e];
+      const T ayw_n = RC.v.v[e] + vCu.v[e], ayw_s = RC.vs.v[e] + vSu.v[e];
+      const T azu = RC.w.v[e] + RE.w.v[e];     // advects u through the top face
+      const T azv = RC.w.v[e] + wN.v[e];
+      const T azw = RC.w.v[e] + wCu.v[e];
+      ry.v[e] = cx * (FW.xx.v[e] - axu * RE.u.v[e]) + cy * (ayu_s * uS.v[e] - ayu_n * uN.v[e]);
+      rv.v[e] = cx * (FW.xy.v[e] - axv * RE.v.v[e]) + cy * (ayv_s * RC.vs.v[e] - ayv_n * vN.v[e]);
+      rwy.v[e] = cx * (FW.xz.v[e] - axw * RE.w.v[e]) + cy * (ayw_s * wS.v[e] - ayw_n * wN.v[e]);
+      FE.xx.v[e] = axu * RC.u.v[e];
+      FE.xy.v[e] = axv * RC.v.v[e];
+      FE.xz.v[e] = axw * RC.w.v[e];
+      su_t.v[e] = azu * uCu.v[e]; pu_t.v[e] = azu * RC.u.v[e];
+      sv_t.v[e] = azv * vCu.v[e]; pv_t.v[e] = azv * RC.v.v[e];
+      sw_t.v[e] = azw * wCu.v[e]; pw_t.v[e] = azw * RC.w.v[e];
+    }
+    const Vec<T> fu_b = shift_down(pu_t, lane, b_xz);
+    const Vec<T> fv_b = shift_down(pv_t, lane, b_yz);
+    const Vec<T> fw_b = shift_down(pw_t, lane, b_zz);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      ou.v[e] = ry.v[e] + (c1.v[e] * fu_b.v[e] - c2.v[e] * su_t.v[e]);
+      ov.v[e] = rv.v[e] + (c1.v[e] * fv_b.v[e] - c2.v[e] * sv_t.v[e]);
+      ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
+    }
+  } else {
+    // six distinct face fluxes (see momentum_step)
+    Vec<T> fyz_n, fzz_t, ry, rv, rwy;
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      const T a = RC.u.v[e] + RE.u.v[e];
+      FE.xx.v[e] = a * a;
+      FE.xy.v[e] = (RC.u.v[e] + uN.v[e]) * (RC.v.v[e] + RE.v.v[e]);
+      const T fxy_se = (uS.v[e] + RC.u.v[e]) * (RC.vs.v[e] + RE.vs.v[e]);
+      FE.xz.v[e] = (RC.u.v[e] + uCu.v[e]) * (RC.w.v[e] + RE.w.v[e]);
+      const T bn = RC.v.v[e] + vN.v[e], bs = RC.vs.v[e] + RC.v.v[e];
+      fyz_n.v[e] = (RC.v.v[e] + vCu.v[e]) * (RC.w.v[e] + wN.v[e]);
+      const T fyz_s = (RC.vs.v[e] + vSu.v[e]) * (wS.v[e] + RC.w.v[e]);
+      const T g = RC.w.v[e] + wCu.v[e];
+      fzz_t.v[e] = g * g;
+      ry.v[e] = cy * (fxy_se - FE.xy.v[e]);
+      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);
+      rv.v[e] = cx * (FW.xy.v[e] - FE.xy.v[e]) + cy * (bs * bs - bn * bn);
+    }
+    const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
+    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
+    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
+      ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
+      ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------
 // tma_momentum<T, ACC>: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks
 // su/sv/sw) from a TMA-fed shared-memory ring.
@@ -261,86 +362,14 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     RE.w = lds_at<0>(pEv + fb, tag);
     const Vec<T> uCu = up_with(RC.u, lds1_at<UP>(pC, tag)), vCu = up_with(RC.v, lds1_at<UP>(pCv, tag));
     const Vec<T> wCu = up_with(RC.w, lds1_at<UP>(pCw, tag)), vSu = up_with(RC.vs, lds1_at<UP>(pCvS, tag));
-    T b_xz = T(0), b_yz = T(0), b_zz = T(0);
+    BelowEdge<T> be;
     if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
-      const T ub = lds1_at<-SZ>(pC, tag), vb = lds1_at<-SZ>(pCv, tag), wb = lds1_at<-SZ>(pCw, tag);
-      const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + nzb, tag);
-      if (SKEW) {
-        b_xz = ub * (wb + web);
-        b_yz = vb * (wb + wnb);
-        b_zz = wb * (wb + RC.w.v[0]);
-      } else {
-        b_xz = (ub + RC.u.v[0]) * (wb + web);
-        b_yz = (vb + RC.v.v[0]) * (wb + wnb);
-        b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
-      }
+      be.ub = lds1_at<-SZ>(pC, tag); be.vb = lds1_at<-SZ>(pCv, tag); be.wb = lds1_at<-SZ>(pCw, tag);
+      be.web = lds1_at<-SZ>(pEv + fb, tag); be.wnb = lds1_at<-SZ>(pCw + nzb, tag);
     }
     Vec<T> ou, ov, ow;
-    if (SKEW) {
-      // Piacsek-Williams skew form (R4): the advected parenthesis holds the
-      // neighbour's value only, so a face carries two products, A*phi_far for the
-      // point on this side and A*phi_near for the point across the face (handed on
-      // through FE in x, by shuffle in z), with the advecting sums A shared.
-      Vec<T> su_t, sv_t, sw_t, pu_t, pv_t, pw_t, ry, rv, rwy;
-#pragma unroll
-      for (int e = 0; e < NK; ++e) {
-        const T axu = RC.u.v[e] + RE.u.v[e];     // advects u through the east face
-        const T axv = RC.u.v[e] + uN.v[e];       // advects v through the east face
-        const T axw = RC.u.v[e] + uCu.v[e];      // advects w through the east face
-        const T ayu_n = RC.v.v[e] + RE.v.v[e], ayu_s = RC.vs.v[e] + RE.vs.v[e];
-        const T ayv_n = RC.v.v[e] + vN.v[e], ayv_s = RC.vs.v[e] + RC.v.v[e];
-        const T ayw_n = RC.v.v[e] + vCu.v[e], ayw_s = RC.vs.v[e] + vSu.v[e];
-        const T azu = RC.w.v[e] + RE.w.v[e];     // advects u through the top face
-        const T azv = RC.w.v[e] + wN.v[e];
-        const T azw = RC.w.v[e] + wCu.v[e];
-        ry.v[e] = cx * (FW.xx.v[e] - axu * RE.u.v[e]) + cy * (ayu_s * uS.v[e] - ayu_n * uN.v[e]);
-        rv.v[e] = cx * (FW.xy.v[e] - axv * RE.v.v[e]) + cy * (ayv_s * RC.vs.v[e] - ayv_n * vN.v[e]);
-        rwy.v[e] = cx * (FW.xz.v[e] - axw * RE.w.v[e]) + cy * (ayw_s * wS.v[e] - ayw_n * wN.v[e]);
-        FE.xx.v[e] = axu * RC.u.v[e];
-        FE.xy.v[e] = axv * RC.v.v[e];
-        FE.xz.v[e] = axw * RC.w.v[e];
-        su_t.v[e] = azu * uCu.v[e]; pu_t.v[e] = azu * RC.u.v[e];
-        sv_t.v[e] = azv * vCu.v[e]; pv_t.v[e] = azv * RC.v.v[e];
-        sw_t.v[e] = azw * wCu.v[e]; pw_t.v[e] = azw * RC.w.v[e];
-      }
-      const Vec<T> fu_b = shift_down(pu_t, lane, b_xz);
-      const Vec<T> fv_b = shift_down(pv_t, lane, b_yz);
-      const Vec<T> fw_b = shift_down(pw_t, lane, b_zz);
-#pragma unroll
-      for (int e = 0; e < NK; ++e) {
-        ou.v[e] = ry.v[e] + (c1.v[e] * fu_b.v[e] - c2.v[e] * su_t.v[e]);
-        ov.v[e] = rv.v[e] + (c1.v[e] * fv_b.v[e] - c2.v[e] * sv_t.v[e]);
-        ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
-      }
-    } else {
-    // six distinct face fluxes (see momentum_step)
-    Vec<T> fyz_n, fzz_t, ry, rv, rwy;
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      const T a = RC.u.v[e] + RE.u.v[e];
-      FE.xx.v[e] = a * a;
-      FE.xy.v[e] = (RC.u.v[e] + uN.v[e]) * (RC.v.v[e] + RE.v.v[e]);
-      const T fxy_se = (uS.v[e] + RC.u.v[e]) * (RC.vs.v[e] + RE.vs.v[e]);
-      FE.xz.v[e] = (RC.u.v[e] + uCu.v[e]) * (RC.w.v[e] + RE.w.v[e]);
-      const T bn = RC.v.v[e] + vN.v[e], bs = RC.vs.v[e] + RC.v.v[e];
-      fyz_n.v[e] = (RC.v.v[e] + vCu.v[e]) * (RC.w.v[e] + wN.v[e]);
-      const T fyz_s = (RC.vs.v[e] + vSu.v[e]) * (wS.v[e] + RC.w.v[e]);
-      const T g = RC.w.v[e] + wCu.v[e];
-      fzz_t.v[e] = g * g;
-      ry.v[e] = cy * (fxy_se - FE.xy.v[e]);
-      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);
-      rv.v[e] = cx * (FW.xy.v[e] - FE.xy.v[e]) + cy * (bs * bs - bn * bn);
-    }
-    const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
-    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
-    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
-      ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
-      ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
-    }
-    }
+    momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, bot_edge, be, c1, c2,
+                            d1, d2, cx, cy, lane, ou, ov, ow);
     if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
     if (last_level) ow.v[NK - 1] = T(0);
     // this warp is done with plane i's slot
@@ -398,6 +427,11 @@ template <typename T>
 struct SqPtrs {
   T *sq[kMaxScalarsPerLaunch];
 };
+// outputs of the momentum role of the fused launch (MOM = true)
+template <typename T>
+struct MomPtrs {
+  T *su, *sv, *sw;
+};
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, int c0, int c1,
                                             int c2, uint32_t bar) {
@@ -441,11 +475,11 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 constexpr int kScalarConsumerWarps = 15;
 constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
 
-template <typename T, int GW, bool ACC, bool SKEW>
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
-            const int nq, const int ngroups, const int gb, const int ty, const int zw,
-            const int ss, const int nstages, const int fieldsz) {
+            const MomPtrs<T> mo, const int nq, const int ngroups, const int gb, const int ty,
+            const int zw, const int ss, const int nstages, const int fieldsz) {
   constexpr int NK = VecOf<T>::NK;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
@@ -471,11 +505,12 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   const int kb0 = zt * ZB;
   const int zlive = min(zw, (nz - kb0 + 32 * NK - 1) / (32 * NK));  // z chunks with a level < nz
   const int slive = (cnt + GW - 1) / GW;                             // splits with a scalar
-  const int ncw = ncol * zlive * slive;                              // live consumer warps
+  const int nr = ss + (MOM ? 1 : 0);                                 // roles per column chunk
+  const int ncw = ncol * zlive * (slive + (MOM ? 1 : 0));            // live consumer warps
   const int i0 = p.ia + blockIdx.y * p.xc;
   const int i1 = min(p.ib, i0 + p.xc);
   const int nplanes = i1 - i0 + 2;  // planes i0-1 .. i1
-  const int nwarps_c = ty * zw * ss;
+  const int nwarps_c = ty * zw * nr;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < nstages; ++s) {
@@ -512,18 +547,102 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   }
 
   // ---------------- consumers ----------------
-  const int col = warp / (zw * ss);
-  const int rem = warp - col * (zw * ss);
-  const int zc = rem / ss;
-  const int sp = rem - zc * ss;
-  if (col >= ncol || zc >= zlive || sp >= slive) return;
-  const int sb = sp * GW;              // first scalar (within the block's group) of this warp
-  const int mycnt = min(GW, cnt - sb);
+  const int col = warp / (zw * nr);
+  const int rem = warp - col * (zw * nr);
+  const int zc = rem / nr;
+  const int sp = rem - zc * nr;
+  if (col >= ncol || zc >= zlive) return;
   const int k0r = kb0 + (zc * 32 + lane) * NK;
   const bool act = k0r < nz;
   const int k0 = act ? k0r : nz - NK;  // clamp: finite data, never stored
   const bool bot_edge = act && lane == 0 && k0 > 0;
   const int e0 = (col + 1) * RS + (k0 - (kb0 - NK));  // element index inside a field tile
+  if (MOM && sp == ss) {
+    // ---------------- momentum role (fused launch): su, sv, sw of this column chunk
+    // from the wind tiles the scalar warps use.  Same x march as tma_momentum; a
+    // plane is read when it lands (as the east plane) and once more one step
+    // later (as the centre plane), so its slot is released one step late.
+    constexpr int SZm = (int)sizeof(T);
+    constexpr int UPm = NK * SZm;
+    const T *const tg = nullptr;
+    const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+    const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
+    const T cx = p.cx, cy = p.cy;
+    const bool first_level = k0 == 0, last_level = k0 + NK == nz;
+    const uint32_t fb = (uint32_t)(fieldsz * SZm), sbytes = (uint32_t)(stagesz * SZm);
+    const uint32_t rsb = (uint32_t)(RS * SZm);
+    const uint32_t a0 = smem_u32(tiles) + (uint32_t)(e0 * SZm);  // u(column, k0) in stage 0
+    const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+    T *qu = mo.su + c0, *qv = mo.sv + c0, *qw = mo.sw + c0;
+    const long long plane = p.plane;
+    pdl_wait();
+    mbar_wait(bar0, 0);  // plane i0-1
+    PlaneRegs<T> RA, RB;
+    XFlux<T> FA, FB;
+    RA.u = lds_at<0>(a0, tg);
+    RA.v = lds_at<0>(a0 + fb, tg);
+    RA.vs = lds_at<0>(a0 + fb - rsb, tg);
+    RA.w = lds_at<0>(a0 + 2 * fb, tg);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
+    int sC = 0, sE = 1 % nstages, t = 0;
+    uint32_t parE = (nstages == 1) ? 1 : 0;
+    uint32_t pC = a0, pE = a0 + (uint32_t)sE * sbytes;
+    const int nsteps = nplanes - 1;
+    auto mstep = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
+      mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
+      const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
+      const Vec<T> uS = lds_at<0>(pC - rsb, tg), uN = lds_at<0>(pC + rsb, tg);
+      const Vec<T> vN = lds_at<0>(pCv + rsb, tg);
+      const Vec<T> wS = lds_at<0>(pCw - rsb, tg), wN = lds_at<0>(pCw + rsb, tg);
+      RE.u = lds_at<0>(pE, tg);
+      RE.v = lds_at<0>(pEv, tg);
+      RE.vs = lds_at<0>(pEv - rsb, tg);
+      RE.w = lds_at<0>(pEv + fb, tg);
+      const Vec<T> uCu = up_with(RC.u, lds1_at<UPm>(pC, tg)), vCu = up_with(RC.v, lds1_at<UPm>(pCv, tg));
+      const Vec<T> wCu = up_with(RC.w, lds1_at<UPm>(pCw, tg));
+      const Vec<T> vSu = up_with(RC.vs, lds1_at<UPm>(pCv - rsb, tg));
+      BelowEdge<T> be;
+      if (bot_edge) {
+        be.ub = lds1_at<-SZm>(pC, tg); be.vb = lds1_at<-SZm>(pCv, tg); be.wb = lds1_at<-SZm>(pCw, tg);
+        be.web = lds1_at<-SZm>(pEv + fb, tg); be.wnb = lds1_at<-SZm>(pCw + rsb, tg);
+      }
+      Vec<T> ou, ov, ow;
+      momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, bot_edge, be, c1,
+                              c2, d1, d2, cx, cy, lane, ou, ov, ow);
+      if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
+      if (last_level) ow.v[NK - 1] = T(0);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));  // done with the centre plane's slot
+      if (t > 0) {
+        if (act) {
+          if (ACC) {
+            const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
+#pragma unroll
+            for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
+          }
+          st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
+        }
+        qu += plane; qv += plane; qw += plane;
+      }
+      sC = sE;
+      pC = pE;
+      pE += sbytes;
+      if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
+      ++t;
+    };
+#pragma unroll 1
+    while (true) {
+      mstep(RA, RB, FA, FB);
+      if (t == nsteps) break;
+      mstep(RB, RA, FB, FA);
+      if (t == nsteps) break;
+    }
+    return;
+  }
+  if (sp >= slive) return;
+  const int sb = sp * GW;              // first scalar (within the block's group) of this warp
+  const int mycnt = min(GW, cnt - sb);
   Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
 #pragma unroll
   for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }

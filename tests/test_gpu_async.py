@@ -96,7 +96,7 @@ def test_step_async_pw_skew():
     hout, hsq = pinned_out(L, 3), pinned_out(L, 4)
     L.step_async(*hin, hq, *hout, hsq)
     L.step_wait()
-    assert "tma_momentum" in L.describe_plan() and "tma_scalars" in L.describe_plan()
+    assert "tma_fused" in L.describe_plan()  # one fused TMA launch per chunk
     for o, w_, n in zip(hout, P.momentum(U, V, W, skew=True), ("su", "sv", "sw")):
         gc.check(cfg, o, w_, n)
         gc.check_halo_untouched(cfg, o, n)

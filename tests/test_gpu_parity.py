@@ -396,3 +396,76 @@ def test_guard_bands(dtype, variant, form):
         g = buf.cpu().numpy()
         assert np.all(g[:G] == gc.SENTINEL) and np.all(g[G + n:] == gc.SENTINEL), f"{nm}: guard written"
     L.close()
+
+
+# ---------------------------------------------------------------------------
+# monc_adv_tendencies: the whole step in one call (fused launch where it fits)
+# ---------------------------------------------------------------------------
+def run_tendencies(cfg, nq, form="flux", fuse=True, tuning=None, accumulate=False):
+    cfgq = dataclasses.replace(cfg, nq=nq)
+    P, L = gc.make_pair(cfgq)
+    L.set_form(form)
+    L.set_fuse(fuse)
+    if tuning:
+        L.set_tuning(**tuning)
+    U, V, W = [synth.field(cfgq, n) for n in "uvw"]
+    names = synth.field_names(cfgq)
+    Q = [synth.field(cfgq, n) for n in names]
+    du, dv, dw = (gc.to_dev(a, L) for a in (U, V, W))
+    dq = [gc.to_dev(a, L) for a in Q]
+    outs = gc.fresh_out(L, 3 + nq)
+    skew = form == "pw_skew"
+    want = list(P.momentum(U, V, W, skew=skew)) + [P.scalar(U, V, W, q, skew=skew) for q in Q]
+    reps = 1
+    if accumulate:
+        for o in outs:
+            h = cfgq.halo
+            o[h:h + cfgq.nx, h:h + cfgq.ny] = 0.0
+        L.set_accumulate(True)
+        reps = 2
+    for _ in range(reps):
+        L.tendencies(du, dv, dw, outs[0], outs[1], outs[2], dq, outs[3:])
+    torch.cuda.synchronize()
+    plan = L.describe_plan()
+    for o, w_, n in zip(outs, want, ["su", "sv", "sw"] + names):
+        gc.check(cfgq, o, reps * w_, n)
+        gc.check_halo_untouched(cfgq, o, n)
+    L.close()
+    return plan
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("form", ["flux", "pw_skew"])
+def test_tendencies_fused(dtype, form):
+    # several y tiles, z tiles and x chunks with ragged tails; every scalar count 1..10
+    cfg = gc.custom_cfg(21, 19, 200, dtype=dtype, cid=310)
+    for nq, tuning in ((1, None), (3, dict(xchunk=8)), (4, dict(xchunk=5, tile_y=2, stages=3)),
+                       (7, dict(xchunk=8, warps=2)), (10, dict(xchunk=6))):
+        plan = run_tendencies(cfg, nq, form=form, tuning=tuning)
+        assert "tma_fused" in plan, plan
+    # nothing to fuse / too many scalars for one group: two launches, same results
+    assert "tma_fused" not in run_tendencies(cfg, 0, form=form)
+    assert "tma_fused" not in run_tendencies(cfg, 11, form=form)
+    assert "tma_fused" not in run_tendencies(cfg, 4, form=form, fuse=False)
+
+
+def test_tendencies_accumulate_and_shapes():
+    run_tendencies(gc.custom_cfg(9, 5, 64, cid=311), 5, accumulate=True)
+    run_tendencies(gc.custom_cfg(3, 1, 4, cid=312), 2)            # ny = 1, one vector per column
+    run_tendencies(gc.custom_cfg(5, 9, 37, cid=313), 2)           # odd nz: generic kernels, two launches
+    run_tendencies(gc.custom_cfg(6, 10, 160, halo=1, cid=314), 4)  # halo 1, 2.5 warps per column
+
+
+def test_tendencies_errors():
+    cfg = gc.custom_cfg(8, 8, 16, nq=2, cid=315)
+    P, L = gc.make_pair(cfg)
+    d = [torch.zeros(L.shape, device="cuda", dtype=L.torch_dtype) for _ in range(5)]
+    o = gc.fresh_out(L, 5)
+    with pytest.raises(binding.MoncAdvError):  # output aliases an input
+        L.tendencies(d[0], d[1], d[2], o[0], o[1], o[2], d[3:], [o[3], d[0]])
+    with pytest.raises(binding.MoncAdvError):  # outputs not distinct
+        L.tendencies(d[0], d[1], d[2], o[0], o[1], o[2], d[3:], [o[3], o[0]])
+    L.tendencies(d[0], d[1], d[2], o[0], o[1], o[2], d[3:], o[3:])
+    L.scalars(d[3:], o[3:])  # the wind is bound by tendencies
+    torch.cuda.synchronize()
+    L.close()
