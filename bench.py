@@ -333,7 +333,7 @@ def run_ours(args):
     fused = None
     if nf > 3 and not args.halo_exchange:
         fsteps = args.steps
-        # the board's power controller averages over ~1 s (DESIGN.md 7.3): let it settle so
+        # the board's power controller averages over ~1 s (DESIGN.md 7.2): let it settle so
         # this loop starts from the same state as the two-call loop above did
         barrier()
         time.sleep(2.0)
