@@ -247,7 +247,7 @@ __device__ __forceinline__ void momentum_faces(
 }
 
 // ---------------------------------------------------------------------------
-// tma_momentum<T, ACC>: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks
+// tma_momentum<T, ACC, SKEW>: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks
 // su/sv/sw) from a TMA-fed shared-memory ring.
 //
 // dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages
@@ -446,7 +446,7 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 }
 
 // ---------------------------------------------------------------------------
-// tma_scalars<GW>: batched scalar tendencies (SURVEY.md 8(a) row a2, 8(c).2
+// tma_scalars<T, GW, ACC, SKEW, MOM>: batched scalar tendencies (SURVEY.md 8(a) row a2, 8(c).2
 // block sq; PAPER.md:83 wind shared by kernels).
 //
 // A block owns a (y, z) tile of `ty` columns x ZB = zw*32*NK levels, advects
@@ -467,6 +467,13 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 // flux differences of plane i (kept in registers as P) and the x flux through
 // the face between planes i-1 and i from the carried q(i-1), u(i-1); with the
 // carried P(i-1) and west flux that completes sq(i-1), which is stored.
+//
+// MOM = true is the fused launch behind monc_adv_tendencies: each
+// column chunk gets one more consumer warp, whose role is the momentum update
+// (su, sv, sw) of that chunk from the SAME staged wind tiles, so u, v, w are
+// read from DRAM once for the whole step.  That warp runs tma_momentum's x march
+// (momentum_faces); it needs a plane twice (east, then centre), so it releases
+// a slot one step after the scalar warps do.  Requires one scalar group.
 //
 // dynamic shared memory: nstages * (3+gb) field tiles of fieldsz elements
 // ((ty+2)*(ZB+2NK) rounded up to 128 B), then 2*nstages mbarriers.
