@@ -149,10 +149,10 @@ def workload_cfg(name):
 # by (workload, kernel family); valid for the library's default launch plan only.
 NCU_TRAFFIC = {
     ("config1", "tma_momentum"): (358.1e6, "profiles/r01_config1_tma_momentum_f64.md"),
-    ("config2", "tma_scalars"): (12970.8e6, "profiles/r01_config2_tma_scalars_f64.md"),
-    ("config3", "tma_scalars"): (6222.6e6, "profiles/r01_config3_tma_f32.md"),
-    ("config2", "tma_fused"): (14240.7e6, "profiles/r01_config2_tma_fused.md"),
-    ("config3", "tma_fused"): (7079.5e6, "profiles/r01_config3_tma_fused.md"),
+    ("config2", "tma_scalars"): (12814.3e6, "profiles/r01_config2_tma_scalars_f64.md"),
+    ("config3", "tma_scalars"): (6206.1e6, "profiles/r01_config3_tma_f32.md"),
+    ("config2", "tma_fused"): (14273.8e6, "profiles/r01_config2_tma_fused.md"),
+    ("config3", "tma_fused"): (7077.1e6, "profiles/r01_config3_tma_fused.md"),
 }
 
 
