@@ -155,7 +155,7 @@ def test_config2_and_3_full_size_sampled(cid):
         # the slab, element by element (columns are independent: PAPER.md:73)
         got = o[sl].cpu().numpy()
         gc.check(slab, got, w_, n + "[slab]")
-    del outs
+    outs_m, scales = outs, [np.abs(gc.interior(slab, w_)).max() for w_ in want_slab]
     # scalars, all nq in one batched call
     outs = gc.fresh_out(L, cfg.nq)
     dq = []
@@ -170,6 +170,21 @@ def test_config2_and_3_full_size_sampled(cid):
         scale = np.abs(gc.interior(slab, w_)).max()
         gc.check_sampled(cfg, P, n, o, U, V, W, Q, ii, jj, kk, scale)
         gc.check(slab, o[sl].cpu().numpy(), w_, n + "[slab]")
+        scales.append(scale)
+    # the whole step through monc_adv_tendencies (the launch bench.py times as the
+    # headline of this config): ONE fused launch, every element within tolerance of the
+    # two-call results just checked against the oracle
+    fo = gc.fresh_out(L, 3 + cfg.nq)
+    L.tendencies(*d, fo[0], fo[1], fo[2], dq, fo[3:])
+    torch.cuda.synchronize()
+    assert "tma_fused" in L.describe_plan(), L.describe_plan()
+    h = cfg.halo
+    for a, b, sc, n in zip(fo, list(outs_m) + list(outs), scales, ["su", "sv", "sw"] + list(names)):
+        ai, bi = (t[h:h + cfg.nx, h:h + cfg.ny] for t in (a, b))
+        err = float((ai - bi).abs().max()) / sc
+        assert err <= gc.TOL[cfg.dtype], f"{n}: fused vs two calls {err:.3e}"
+        gc.check_sampled(cfg, P, n if n in ("su", "sv", "sw") else n, a, U, V, W,
+                         None if n in ("su", "sv", "sw") else synth.field(cfg, n), ii, jj, kk, sc)
     L.close()
 
 
