@@ -195,8 +195,8 @@ int monc_adv_set_variant(monc_adv_t h, int variant);
  *   group:    scalars that share one staged copy of the wind: per thread block
  *             (1..10) in variant 3, per thread (1..5) in variant 2;
  *   prefetch: L2 prefetch distance in planes (-1 = no prefetch), variant 2;
- *   warps:    variant 2: warps per thread block (1..8); variant 3 scalars:
- *             32-vector z chunks per thread block;
+ *   warps:    variant 2: warps per thread block (1..8); ignored by variant 3 (a
+ *             block tile is one 32-vector z chunk per column);
  *   stages:   depth of the TMA ring (2..8), variant 3;
  *   tile_y:   columns per thread block, variant 3;
  *   split:    variant 3 scalars: warps that share one column chunk and split

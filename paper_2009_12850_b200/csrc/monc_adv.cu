@@ -114,17 +114,21 @@ int pick_xchunk(monc_adv_t h, int nplanes, int blocks_per_plane, int resident_pe
 // takes.  Measured on B200: a GPC sustains about 16 SMs' worth
 // of these streaming kernels.  Up to 8 x 16 = 128 blocks run at the full per-SM
 // rate; a single static wave of 129..148 blocks is as slow as its fullest GPC
-// (20 SMs on 16 SMs' worth of bandwidth: 1.27 x at 148 blocks); many waves are
-// balanced dynamically (about 1.12 block-times per 148 blocks), and a partial
-// last wave costs a whole block-time again.
+// (20 SMs on 16 SMs' worth of bandwidth: 1.27 x at 148 blocks).  Several waves of
+// short blocks are balanced dynamically: about 1.12 block-times per 148 blocks,
+// plus half a block-time for the ragged end.  A single wave that leaves SMs idle
+// is charged for them (0.95 x SMs / blocks): under the board's power cap the SM
+// clock drops and the per-SM rate, not DRAM, bounds the launch (config 2 momentum,
+// 128 blocks x 512 planes against 1024 x 64: 4 % faster in a burst, 6 % slower
+// sustained).
 double launch_rounds(long blocks, int sm_count) {
   const long full_rate = std::max(1L, (long)sm_count * 128 / 148);
-  auto one_wave = [&](long b) {
-    return b <= full_rate ? 1.0 : 1.0 + 0.27 * (double)(b - full_rate) / (double)(sm_count - full_rate);
-  };
-  if (blocks <= sm_count) return one_wave(blocks);
-  const long full = blocks / sm_count, rem = blocks % sm_count;
-  return 1.12 * full + (rem ? one_wave(rem) : 0.0);
+  const double idle = 0.95 * (double)sm_count / (double)std::max(1L, blocks);
+  if (blocks <= full_rate) return std::max(1.0, idle);
+  if (blocks <= sm_count)
+    return std::max(idle, 1.0 + 0.27 * (double)(blocks - full_rate) / (double)(sm_count - full_rate));
+  if (blocks < 2L * sm_count) return 1.12 + 1.0;  // one full wave and a partial one, each a whole block-time
+  return 1.12 * (double)blocks / (double)sm_count + 0.5;
 }
 
 // geometry of the TMA-staged kernels: TY columns per block, ring depth S
@@ -159,10 +163,11 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
       // time ~ block-times of the launch * (columns per block + the L2/shared-memory
-      // cost of its two halo columns) * (planes per block + its two halo planes)
+      // cost of its two halo columns) * (planes per block + its two halo planes + the
+      // ramp of a deep ring)
       const double rounds = launch_rounds(blocks, h->sm_count);
       const double march = 1.0 + 0.1 * std::min(xc, 256) / 256.0;  // y neighbours drift apart
-      const double cost = rounds * (ty + 0.7) * (xc + 2) * (1.0 + 0.02 * (tymax - ty)) * march;
+      const double cost = rounds * (ty + 0.7) * (xc + 4) * (1.0 + 0.02 * (tymax - ty)) * march;
       if (cost < best) {
         best = cost;
         pl.ok = true; pl.ty = ty; pl.stages = S; pl.xc = xc; pl.tiles = tiles;
@@ -292,7 +297,6 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
   const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
   const int wzc = (h->nz / NK + 31) / 32;  // warps a whole column needs
   const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
-  const int zwmax = std::min({wzc, kScalarConsumerWarps, (256 - 2 * NK) / (32 * NK)});  // box dim <= 256
   double best = 1e300;
   // Cost model, calibrated on B200:
   // a block step (one plane) takes max(DRAM time of its bytes at this SM's share
@@ -309,9 +313,9 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
       if (h->split > 0 && ss != std::min(h->split, std::min(gb, 4))) continue;
       const int gw = (gb + ss - 1) / ss;
       if (gw > 5) continue;
-      for (int zw = 1; zw <= zwmax; ++zw) {
-        if (h->warps > 0 && zw != std::min(h->warps, zwmax)) continue;
-        const int ZB = zw * 32 * NK, RS = ZB + 2 * NK;
+      {
+        constexpr int zw = 1;  // one 32-vector z chunk per block tile: the row stride is a compile-time constant
+        const int ZB = 32 * NK, RS = kRowBytes / (int)sizeof(T);
         const int nzt = (h->nz + ZB - 1) / ZB;
         const int tymax = std::min(h->ny, kScalarConsumerWarps / (zw * (ss + (mom ? 1 : 0))));
         if (tymax < 1) continue;
@@ -336,11 +340,12 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
             const int xc = (nplanes + nch - 1) / nch;
             const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);
             const double waves = launch_rounds(blocks, h->sm_count);
-            // +2 halo planes, ~2 steps of start-up latency; on a long march the y/z
-            // neighbours drift apart and their halo re-reads miss L2 (config 2: DRAM
-            // reads 8.9 GB at xc = 512 against 7.7 GB at xc = 64, 11 % slower)
-            const double march = 1.0 + 0.2 * std::min(xc, 512) / 512.0;
-            const double cost = waves * (xc + (waves <= 1.3 ? 4 : 2)) * t_step * march;
+            // +2 halo planes, ~1-2 steps of start-up latency; on a long march the y/z
+            // neighbours drift apart (the SMs of a full GPC get less bandwidth each) and
+            // their halo re-reads miss L2: config 2 fused, DRAM reads 7.95 GB at xc = 103
+            // against 7.09 GB algorithmic; 5 % faster at xc = 32..52
+            const double march = 1.0 + 0.0007 * std::min(xc, 512);
+            const double cost = waves * (xc + (waves <= 1.3 ? 4 : 3)) * t_step * march;
             if (cost < best) {
               best = cost;
               pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
@@ -365,7 +370,7 @@ int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &ma
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * pl.zw * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
   CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
-                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.zw, pl.ss, pl.stages, pl.fieldsz));
+                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
 }
 
@@ -405,7 +410,7 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
       if (base == 0) return MONC_ADV_OK;
       return fail(h, MONC_ADV_ECUDA, "scalars: TMA plan failed after a partial launch");
     }
-    const int RS = pl.zw * 32 * NK + 2 * NK;
+    const int RS = kRowBytes / (int)sizeof(T);
     TensorMaps maps;
     SqPtrs<T> outs;
     bool ok = encode_field_map<T>(h, &maps.m[0], u, RS, pl.ty + 2) &&

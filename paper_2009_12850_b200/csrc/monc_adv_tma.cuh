@@ -1,23 +1,25 @@
-// monc_adv_tma.cuh -- TMA-staged variants of the marching kernels (sm_100a).
+// monc_adv_tma.cuh -- TMA-staged x-marching kernels (sm_100a): the default path.
 //
-// Same arithmetic as march_momentum / march_scalars (momentum_step is shared),
-// different data movement: a thread block owns TY full columns (+1 halo column
-// on each side) and marches a chunk of x planes.  At fixed x such a tile is ONE
-// contiguous run of (TY+2)*nz elements per field in MONC's z-fastest layout,
-// so a single producer lane streams plane after plane into a shared-memory
-// ring with 1-D bulk TMA copies (cp.async.bulk, SASS UBLKCP) that complete on
-// mbarriers, running several planes ahead of the consumers.  DRAM latency is
-// hidden by the ring depth instead of by registers or occupancy; y neighbours
-// and z-chunk edges are plain shared-memory reads.  There is no dedicated
-// producer warp (a 17th warp would cap the block at 96 registers per thread):
-// lane 0 of the last warp refills, one step late, the slot every warp has
-// released, so the ring runs nstages-2 planes ahead.
+// Data movement.  A thread block owns a y tile of full or partial columns and
+// marches a chunk of x planes.  At fixed x such a tile is staged into a ring of
+// shared-memory slots by the TMA unit (tma_momentum: ONE contiguous 1-D bulk
+// copy per field per plane, cp.async.bulk / SASS UBLKCP; tma_scalars: ONE
+// tensor-map box copy per field per plane, cp.async.bulk.tensor / UTMALDG),
+// completing on mbarriers and running several planes ahead of the consumers.
+// DRAM latency is hidden by the ring depth instead of by occupancy; y
+// neighbours and z-chunk edges are plain shared-memory reads, vertical face
+// fluxes travel between lanes by warp shuffle, x-face fluxes are carried in
+// registers from one plane to the next, so every face flux is computed once.
+//
+// The x march of the fused momentum update exists ONCE (momentum_march): it is
+// the consumer loop of tma_momentum and the momentum role of the fused launch.
 #pragma once
 #include "monc_adv_kernels.cuh"
 
 #include <cuda.h>  // CUtensorMap (type only; the encoder is fetched at run time)
 
 #include <cstdint>
+#include <type_traits>
 
 namespace monc {
 
@@ -69,29 +71,6 @@ __device__ __forceinline__ void pdl_launch_dependents() {
 }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-__device__ __forceinline__ Vec<double> lds_vec(const double *p) {
-  const double2 t = *reinterpret_cast<const double2 *>(p);
-  Vec<double> r;
-  r.v[0] = t.x; r.v[1] = t.y;
-  return r;
-}
-__device__ __forceinline__ Vec<float> lds_vec(const float *p) {
-  const float4 t = *reinterpret_cast<const float4 *>(p);
-  Vec<float> r;
-  r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
-  return r;
-}
-// r[e] = a[e+1], last element read from shared memory (level k0 + NK)
-template <typename T>
-__device__ __forceinline__ Vec<T> up_from_smem(const Vec<T> &a, const T *next) {
-  constexpr int NK = VecOf<T>::NK;
-  Vec<T> r;
-#pragma unroll
-  for (int e = 0; e + 1 < NK; ++e) r.v[e] = a.v[e + 1];
-  r.v[NK - 1] = *next;
-  return r;
-}
-
 // ---------------------------------------------------------------------------
 // Shared-memory loads by 32-bit shared-window address with a compile-time byte
 // offset folded into the instruction ([R + imm]): the consumers' address
@@ -132,6 +111,24 @@ __device__ __forceinline__ Vec<T> up_with(const Vec<T> &a, const T top) {
   r.v[NK - 1] = top;
   return r;
 }
+// r[e] = a[e-1]; the first element is the scalar `bot` (level k0 - 1)
+template <typename T>
+__device__ __forceinline__ Vec<T> down_with(const Vec<T> &a, const T bot) {
+  constexpr int NK = VecOf<T>::NK;
+  Vec<T> r;
+#pragma unroll
+  for (int e = 1; e < NK; ++e) r.v[e] = a.v[e - 1];
+  r.v[0] = bot;
+  return r;
+}
+// x & m bit by bit (m = 0 or ~0): forces an exact +0 without a predicate, so the
+// "no tendency at this level" rule costs a logic op instead of a compare + select
+__device__ __forceinline__ double keep_if(double x, int m) {
+  return __hiloint2double(__double2hiint(x) & m, __double2loint(x) & m);
+}
+__device__ __forceinline__ float keep_if(float x, int m) {
+  return __int_as_float(__float_as_int(x) & m);
+}
 
 // values of one x plane a thread carries to the next x step: u, v, w at its
 // column and v at the column to the south
@@ -145,40 +142,23 @@ struct XFlux {
   Vec<T> xx, xy, xz;
 };
 
-// the values one level below a warp's first level (lane 0 of the upper z chunks)
-template <typename T>
-struct BelowEdge {
-  T ub, vb, wb, web, wnb;  // u, v, w of the centre plane; w of the east plane and of the north column
-};
-
 // ---------------------------------------------------------------------------
 // One x step of the fused momentum update for a thread's NK levels (SURVEY.md
 // 8(c).2 blocks su/sv/sw): centre plane RC, east plane RE, the centre plane's
 // south/north/upper neighbours, the west-face terms FW carried from the
-// previous step.  Returns the tendencies of the centre plane and, in FE, the
-// east-face terms the next step needs as its west.
+// previous step, and the three vertical fluxes b_* through the face below the
+// thread's first level that a shuffle cannot provide (lane 0; unused elsewhere).
+// Returns the tendencies of the centre plane and, in FE, the east-face terms
+// the next step needs as its west.
 // ---------------------------------------------------------------------------
 template <typename T, bool SKEW>
 __device__ __forceinline__ void momentum_faces(
     const PlaneRegs<T> &RC, const PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE,
     const Vec<T> &uS, const Vec<T> &uN, const Vec<T> &vN, const Vec<T> &wS, const Vec<T> &wN,
-    const Vec<T> &uCu, const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const bool bot_edge,
-    const BelowEdge<T> &be, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1, const Vec<T> &d2,
+    const Vec<T> &uCu, const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const T b_xz,
+    const T b_yz, const T b_zz, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1, const Vec<T> &d2,
     const T cx, const T cy, const int lane, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
   constexpr int NK = VecOf<T>::NK;
-  T b_xz = T(0), b_yz = T(0), b_zz = T(0);
-  if (bot_edge) {
-    const T ub = be.ub, vb = be.vb, wb = be.wb, web = be.web, wnb = be.wnb;
-    if (SKEW) {
-      b_xz = ub * (wb + web);
-      b_yz = vb * (wb + wnb);
-      b_zz = wb * (wb + RC.w.v[0]);
-    } else {
-      b_xz = (ub + RC.u.v[0]) * (wb + web);
-      b_yz = (vb + RC.v.v[0]) * (wb + wnb);
-      b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
-    }
-  }
   if (SKEW) {
     // Piacsek-Williams skew form (R4): the advected parenthesis holds the
     // neighbour's value only, so a face carries two products, A*phi_far for the
@@ -216,7 +196,10 @@ __device__ __forceinline__ void momentum_faces(
       ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
     }
   } else {
-    // six distinct face fluxes (see momentum_step)
+    // six distinct face fluxes:
+    //   fxx (u_i+u_i+1)^2            fyy (v_j+v_j+1)^2           fzz (w_K+w_K+1)^2
+    //   fxy (u_j+u_j+1)(v_i+v_i+1)   fxz (u_K+u_K+1)(w_i+w_i+1)  fyz (v_K+v_K+1)(w_j+w_j+1)
+    // (FyU == FxV, FzU == FxW, FzV == FyW up to the constant)
     Vec<T> fyz_n, fzz_t, ry, rv, rwy;
 #pragma unroll
     for (int e = 0; e < NK; ++e) {
@@ -247,13 +230,141 @@ __device__ __forceinline__ void momentum_faces(
 }
 
 // ---------------------------------------------------------------------------
+// momentum_march: the x march of one warp over its column chunk, fed by a ring
+// of staged planes.  Used by tma_momentum (every consumer warp) and by the
+// momentum role of the fused launch (tma_scalars<.., MOM = true>).
+//
+// Ring protocol: full[s] at bar0 + 8 s completes when the plane in slot s has
+// landed; the warp reads a plane when it lands (as the east plane; the values
+// it needs again stay in registers) and once more one step later (as the centre
+// plane: south/north/upper neighbours), then releases the slot with ONE arrival
+// (lane 0) on empty[s] at bar0 + 8 (nstages + s).  `after_release()` runs right
+// after that arrival in every step but the first (tma_momentum's refilling lane;
+// nothing in the fused launch).
+//
+// Slot layout, in bytes: field f of stage s at s * sbytes + f * fb, rows rsb
+// apart; a0 = shared address of u(this column, k0) in stage 0.  The x loop is
+// unrolled by two with the register sets of the centre and east planes (and of
+// the west/east x fluxes) swapping roles, so the plane rotation costs no moves.
+// ---------------------------------------------------------------------------
+template <typename T>
+struct MarchArgs {
+  uint32_t a0, fb, sbytes, rsb, bar0;
+  int nstages, nsteps, lane;
+  bool act, bot_edge;
+  bool first_level, last_level;  // element 0 is level K = 1 (no tendency) / element NK-1 is level K = nz (sw = 0)
+  T *su, *sv, *sw;            // output arrays (kernel parameters: re-read from the constant bank, not kept in registers)
+  long long c0, plane;        // element offset of (i0, j, k0); elements per x plane
+  T cx, cy;
+  Vec<T> c1, c2, d1, d2;
+};
+
+template <typename T, bool ACC, bool SKEW, typename AfterRelease>
+__device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelease &&after_release) {
+  constexpr int NK = VecOf<T>::NK;
+  constexpr int SZ = (int)sizeof(T);
+  constexpr int UP = NK * SZ;  // byte offset of the level above a vector's last element
+  const T *const tag = nullptr;
+  const uint32_t a0 = m.a0, fb = m.fb, sbytes = m.sbytes, rsb = m.rsb, bar0 = m.bar0;
+  const int nstages = m.nstages, lane = m.lane;
+  const bool bot_edge = m.bot_edge;
+  long long c = m.c0;
+
+  mbar_wait(bar0, 0);  // plane i0-1
+  PlaneRegs<T> RA, RB;
+  XFlux<T> FA, FB;
+  RA.u = lds_at<0>(a0, tag);
+  RA.v = lds_at<0>(a0 + fb, tag);
+  RA.vs = lds_at<0>(a0 + fb - rsb, tag);
+  RA.w = lds_at<0>(a0 + 2 * fb, tag);
+#pragma unroll
+  for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
+
+  int sC = 0, sE = 1 % nstages;
+  uint32_t parE = (nstages == 1) ? 1 : 0;
+  uint32_t pC = a0, pE = a0 + (uint32_t)sE * sbytes;
+
+  // one x step: centre plane in RC (registers) / stage sC, east plane arriving in stage sE.
+  // The first step (plane i0-1 as the centre) only builds the x-face terms: no store.
+  bool first = true;
+  auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
+    mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
+    const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
+    const Vec<T> uS = lds_at<0>(pC - rsb, tag), uN = lds_at<0>(pC + rsb, tag);
+    const Vec<T> vN = lds_at<0>(pCv + rsb, tag);
+    const Vec<T> wS = lds_at<0>(pCw - rsb, tag), wN = lds_at<0>(pCw + rsb, tag);
+    RE.u = lds_at<0>(pE, tag);
+    RE.v = lds_at<0>(pEv, tag);
+    RE.vs = lds_at<0>(pEv - rsb, tag);
+    RE.w = lds_at<0>(pEv + fb, tag);
+    const Vec<T> uCu = up_with(RC.u, lds1_at<UP>(pC, tag)), vCu = up_with(RC.v, lds1_at<UP>(pCv, tag));
+    const Vec<T> wCu = up_with(RC.w, lds1_at<UP>(pCw, tag));
+    const Vec<T> vSu = up_with(RC.vs, lds1_at<UP>(pCv - rsb, tag));
+    T b_xz = T(0), b_yz = T(0), b_zz = T(0);
+    if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
+      const T ub = lds1_at<-SZ>(pC, tag), vb = lds1_at<-SZ>(pCv, tag), wb = lds1_at<-SZ>(pCw, tag);
+      const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + rsb, tag);
+      if (SKEW) {
+        b_xz = ub * (wb + web);
+        b_yz = vb * (wb + wnb);
+        b_zz = wb * (wb + RC.w.v[0]);
+      } else {
+        b_xz = (ub + RC.u.v[0]) * (wb + web);
+        b_yz = (vb + RC.v.v[0]) * (wb + wnb);
+        b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
+      }
+    }
+    Vec<T> ou, ov, ow;
+    momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, m.c1,
+                            m.c2, m.d1, m.d2, m.cx, m.cy, lane, ou, ov, ow);
+    // this warp is done with the centre plane's slot
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
+    if (!first) {
+      after_release();
+      if (m.first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
+      if (m.last_level) ow.v[NK - 1] = T(0);
+      if (m.act) {
+        T *qu = m.su + c, *qv = m.sv + c, *qw = m.sw + c;
+        if (ACC) {
+          const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
+#pragma unroll
+          for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
+        }
+        st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
+      }
+      c += m.plane;
+    }
+    first = false;
+    sC = sE;
+    pC = pE;
+    pE += sbytes;
+    if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
+  };
+  int left = m.nsteps;
+#pragma unroll 1
+  while (true) {
+    step(RA, RB, FA, FB);
+    if (--left == 0) break;
+    step(RB, RA, FB, FA);
+    if (--left == 0) break;
+  }
+}
+
+// ---------------------------------------------------------------------------
 // tma_momentum<T, ACC, SKEW>: fused su, sv, sw (SURVEY.md 8(a) row a1, 8(c).2 blocks
 // su/sv/sw) from a TMA-fed shared-memory ring.
 //
+// One block = `ty` full columns x a chunk of xc planes; warp <-> (column, 32-vector
+// z chunk).  A stage holds the u, v, w tiles of one plane, rows [jr0-1, jr0+ty]:
+// at fixed x that is ONE contiguous run of (ty+2)*nz elements per field, so one
+// 1-D bulk copy per field fills it.  There is no dedicated producer warp (a 17th
+// warp would cap the block at 96 registers per thread): lane 0 of the last warp
+// refills, one step late, the slot every warp has released, so the ring runs
+// nstages-2 planes ahead.
+//
 // dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages
-// mbarriers.  The x loop is unrolled by two with the register sets of the
-// centre and east planes (and of the west/east x fluxes) swapping roles, so
-// the plane rotation costs no register moves.
+// mbarriers.
 // ---------------------------------------------------------------------------
 template <typename T, bool ACC, bool SKEW>
 __global__ void __launch_bounds__(kTmaThreads, 1)
@@ -262,8 +373,6 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
              T *__restrict__ sv, T *__restrict__ sw) {
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
-  constexpr int UP = NK * SZ;  // byte offset of the level above a vector's last element
-  const T *const tag = nullptr;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -294,18 +403,19 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   const int col = warp / p.wzc;
   const int zc = warp - col * p.wzc;
   const int k0r = (zc * 32 + lane) * NK;
-  const bool act = k0r < nz;
-  const int k0 = act ? k0r : nz - NK;
-  const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
-  const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
+  MarchArgs<T> m;
+  m.act = k0r < nz;
+  const int k0 = m.act ? k0r : nz - NK;  // clamp: finite data, never stored
+  m.c1 = ld_vec(p.tzc1 + k0); m.c2 = ld_vec(p.tzc2 + k0);
+  m.d1 = ld_vec(p.tzd1 + k0); m.d2 = ld_vec(p.tzd2 + k0);
   pdl_wait();  // the fields may have been written by the previous kernel in the stream
   // ---------------- producer role: lane 0 of the last warp ----------------
   const bool producer = (warp == ncw - 1) && lane == 0;
   const uint32_t tile_bytes = (uint32_t)((ncol + 2) * nz * SZ);
   const uint32_t t0 = smem_u32(tiles);
-  const uint32_t fb = (uint32_t)(fieldsz * SZ), sb = 3u * fb, nzb = (uint32_t)(nz * SZ);
+  const uint32_t fb = (uint32_t)(fieldsz * SZ), sb = 3u * fb;
   long long g_next = ((long long)(i0 - 1) * p.nyh + (jr0 + p.h - 1)) * nz;  // next plane to load
-  int pl_next = 0, s_next = 0;
+  int to_issue = nsteps + 1, s_next = 0;  // planes i0-1 .. i1
   uint32_t par_next = 0;  // parity of the empty-phase the next refill of slot s_next waits for
   auto issue_plane = [&]() {
     const uint32_t full = bar0 + 8 * s_next;
@@ -315,107 +425,40 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     tma_load_1d(dst + fb, v + g_next, tile_bytes, full);
     tma_load_1d(dst + 2 * fb, w + g_next, tile_bytes, full);
     g_next += p.plane;
-    ++pl_next;
+    --to_issue;
     if (++s_next == nstages) s_next = 0;
   };
   if (producer) {
-    const int first = min(nstages, nsteps + 1);  // planes i0-1 .. i1 = nsteps + 1 planes
+    const int first = min(nstages, nsteps + 1);
     for (int n = 0; n < first; ++n) issue_plane();
   }
 
   // ---------------- consumers: warp <-> (column, z chunk) ----------------
-  const bool bot_edge = act && lane == 0 && zc > 0;
-  const bool first_level = k0 == 0;        // element 0 is level K = 1: no tendency
-  const bool last_level = k0 + NK == nz;   // element NK-1 is level K = nz: sw = 0
-  const T cx = p.cx, cy = p.cy;
-  const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
-  T *qu = su + c0, *qv = sv + c0, *qw = sw + c0;
-  const long long plane = p.plane;
-  const uint32_t a0 = t0 + (uint32_t)(((col + 1) * nz + k0) * SZ);  // u(column, k0) in stage 0
-
-  mbar_wait(bar0, 0);  // plane i0-1
-  PlaneRegs<T> RA, RB;
-  XFlux<T> FA, FB;
-  RA.u = lds_at<0>(a0, tag);
-  RA.v = lds_at<0>(a0 + fb, tag);
-  RA.vs = lds_at<0>(a0 + fb - nzb, tag);
-  RA.w = lds_at<0>(a0 + 2 * fb, tag);
-#pragma unroll
-  for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
-
-  int sC = 0, sE = 1 % nstages;
-  uint32_t parE = (nstages == 1) ? 1 : 0;
-  uint32_t pC = a0, pE = a0 + (uint32_t)sE * sb;
-  int t = 0;
-
-  // one x step: centre plane in RC (registers) / stage sC, east plane arriving in stage sE
-  auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
-    mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
-    const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
-    const uint32_t pCuS = pC - nzb, pCvS = pCv - nzb, pCwS = pCw - nzb;
-    const Vec<T> uS = lds_at<0>(pCuS, tag), uN = lds_at<0>(pC + nzb, tag);
-    const Vec<T> vN = lds_at<0>(pCv + nzb, tag);
-    const Vec<T> wS = lds_at<0>(pCwS, tag), wN = lds_at<0>(pCw + nzb, tag);
-    RE.u = lds_at<0>(pE, tag);
-    RE.v = lds_at<0>(pEv, tag);
-    RE.vs = lds_at<0>(pEv - nzb, tag);
-    RE.w = lds_at<0>(pEv + fb, tag);
-    const Vec<T> uCu = up_with(RC.u, lds1_at<UP>(pC, tag)), vCu = up_with(RC.v, lds1_at<UP>(pCv, tag));
-    const Vec<T> wCu = up_with(RC.w, lds1_at<UP>(pCw, tag)), vSu = up_with(RC.vs, lds1_at<UP>(pCvS, tag));
-    BelowEdge<T> be;
-    if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
-      be.ub = lds1_at<-SZ>(pC, tag); be.vb = lds1_at<-SZ>(pCv, tag); be.wb = lds1_at<-SZ>(pCw, tag);
-      be.web = lds1_at<-SZ>(pEv + fb, tag); be.wnb = lds1_at<-SZ>(pCw + nzb, tag);
-    }
-    Vec<T> ou, ov, ow;
-    momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, bot_edge, be, c1, c2,
-                            d1, d2, cx, cy, lane, ou, ov, ow);
-    if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
-    if (last_level) ow.v[NK - 1] = T(0);
-    // this warp is done with plane i's slot
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
-    if (producer && t >= 1 && pl_next <= nsteps) {
+  m.a0 = t0 + (uint32_t)(((col + 1) * nz + k0) * SZ);  // u(column, k0) in stage 0
+  m.fb = fb; m.sbytes = sb; m.rsb = (uint32_t)(nz * SZ); m.bar0 = bar0;
+  m.nstages = nstages; m.nsteps = nsteps; m.lane = lane;
+  m.bot_edge = m.act && lane == 0 && zc > 0;
+  m.first_level = k0 == 0;
+  m.last_level = k0 + NK == nz;
+  m.c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+  m.su = su; m.sv = sv; m.sw = sw;
+  m.plane = p.plane;
+  m.cx = p.cx; m.cy = p.cy;
+  momentum_march<T, ACC, SKEW>(m, [&]() {
+    if (producer && to_issue > 0) {
       // slot of plane i-1: every warp released it during the previous step
       mbar_wait(bar0 + 8 * (nstages + s_next), par_next);
       issue_plane();
       if (s_next == 0) par_next ^= 1;
     }
-    if (t > 0) {
-      if (act) {
-        if (ACC) {
-          const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
-#pragma unroll
-          for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
-        }
-        st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
-      }
-      qu += plane; qv += plane; qw += plane;
-    }
-    sC = sE;
-    pC = pE;
-    pE += sb;
-    if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
-    ++t;
-  };
-#pragma unroll 1
-  while (true) {
-    step(RA, RB, FA, FB);
-    if (t == nsteps) break;
-    step(RB, RA, FB, FA);
-    if (t == nsteps) break;
-  }
+  });
 }
-
-}  // namespace monc
-
-namespace monc {
 
 // ---------------------------------------------------------------------------
 // Tensor-map TMA (cp.async.bulk.tensor, SASS UTMALDG): one instruction moves a
 // (z, y) box of one x plane of one field, strided rows and all, and fills
 // out-of-range elements (levels below 0 / above nz-1, rows past the array)
-// with zeros.  Descriptors are encoded on the host per call (the field
+// with zeros.  Descriptors are encoded on the host per plan (the field
 // pointers are call arguments) and passed as __grid_constant__ parameters.
 // ---------------------------------------------------------------------------
 constexpr int kMaxScalarsPerLaunch = 20;  // 23 descriptors of 128 B stay below the 4 KB parameter limit
@@ -449,54 +492,182 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 // tma_scalars<T, GW, ACC, SKEW, MOM>: batched scalar tendencies (SURVEY.md 8(a) row a2, 8(c).2
 // block sq; PAPER.md:83 wind shared by kernels).
 //
-// A block owns a (y, z) tile of `ty` columns x ZB = zw*32*NK levels, advects
-// gb = GW*ss scalars of one group and marches a chunk of x planes.  A stage of
-// the ring holds, for u, v, w and the gb scalars, the box rows [jr0-1, jr0+ty]
-// x levels [kb0-NK, kb0+ZB+NK) of ONE plane: one tensor-map TMA copy per field,
-// issued by a dedicated producer warp (lanes 0..2+gb), completing on the
-// stage's `full` mbarrier.  Elements outside the array are zero-filled by the
-// TMA unit: they are read (the top level's upper neighbour) but multiplied by
-// a zero coefficient.
+// A block owns a (y, z) tile of `ty` columns x ZB = 32*NK levels (one 16-byte
+// vector per lane), advects gb = GW*ss scalars of one group and marches a chunk of
+// x planes.  A stage of the ring holds, for u, v, w and the gb scalars, the box
+// rows [jr0-1, jr0+ty] x levels [kb0-NK, kb0+ZB+NK) of ONE plane: one tensor-map
+// TMA copy per field, issued by a dedicated producer warp (lanes 0..2+gb),
+// completing on the stage's `full` mbarrier.  Elements outside the array are
+// zero-filled by the TMA unit: they are read (the top level's upper neighbour)
+// but multiplied by a zero coefficient.  The row stride is the compile-time
+// constant kRowBytes = 34 vectors for both dtypes, so the y and z neighbours of
+// a value are immediate offsets from one register.
 //
-// Consumer warp <-> (column, 32-vector z chunk, scalar split): `ss` warps share
-// one column chunk and take GW scalars each, so the warp count (latency hiding)
-// does not shrink when the tile is made small enough for a deep ring.
+// Consumer warp <-> (column, scalar split): `ss` warps share one column chunk
+// and take GW scalars each, so the warp count (latency hiding) does not shrink
+// when the tile is made small enough for a deep ring.
 //
 // Every plane is touched in exactly ONE consumer step (so S-1 of the S stages
-// can be in flight): when plane i lands a thread forms, per scalar, the y and z
-// flux differences of plane i (kept in registers as P) and the x flux through
-// the face between planes i-1 and i from the carried q(i-1), u(i-1); with the
-// carried P(i-1) and west flux that completes sq(i-1), which is stored.
+// can be in flight).  When plane i lands a thread forms, once for its GW scalars,
+// the advecting velocities of the four faces of plane i scaled by their
+// coefficients (2cx u, 2cy v, 2tzc1 w below, 2tzc2 w) and then, per scalar, the y
+// and z flux differences P of plane i and the x flux f through the face between
+// planes i-1 and i: A = P + f is carried to the next step, where subtracting that
+// step's f completes sq(i), which is stored.  Two values per scalar stay in
+// registers from one plane to the next (q and A).
 //
 // MOM = true is the fused launch behind monc_adv_tendencies: each
 // column chunk gets one more consumer warp, whose role is the momentum update
-// (su, sv, sw) of that chunk from the SAME staged wind tiles, so u, v, w are
-// read from DRAM once for the whole step.  That warp runs tma_momentum's x march
-// (momentum_faces); it needs a plane twice (east, then centre), so it releases
-// a slot one step after the scalar warps do.  Requires one scalar group.
+// (su, sv, sw) of that chunk from the SAME staged wind tiles (momentum_march), so
+// u, v, w are read from DRAM once for the whole step.  It needs a plane twice
+// (east, then centre), so it releases a slot one step after the scalar warps do.
+// Requires one scalar group.
 //
 // dynamic shared memory: nstages * (3+gb) field tiles of fieldsz elements
-// ((ty+2)*(ZB+2NK) rounded up to 128 B), then 2*nstages mbarriers.
+// ((ty+2) rows of kRowBytes, rounded up to 128 B), then 2*nstages mbarriers.
 // ---------------------------------------------------------------------------
 // 15 consumer warps + the producer warp = 512 threads: 128 registers per thread
 constexpr int kScalarConsumerWarps = 15;
 constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
+constexpr int kRowBytes = 34 * 16;  // 32 vectors of the tile + one vector of z halo on each side
+
+// The scalar role of one warp: GW scalars (mycnt of them live when !FULL) of one
+// column chunk over the block's planes.
+template <typename T, int GW, bool ACC, bool SKEW, bool FULL>
+__device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t fb, const uint32_t sbytes,
+                                             const uint32_t q0off, const uint32_t bar0, const int nstages,
+                                             const int nplanes, const int mycnt, const int lane,
+                                             const bool act, const bool bot_edge, const int keep_first,
+                                             T *const *__restrict__ sqp, const long long c0,
+                                             const long long plane, const Vec<T> &c1, const Vec<T> &c2,
+                                             const T cx2, const T cy2) {
+  constexpr int NK = VecOf<T>::NK;
+  constexpr int SZ = (int)sizeof(T);
+  constexpr int UP = NK * SZ;
+  constexpr int RSB = kRowBytes;
+  const T *const tag = nullptr;
+  // carried per scalar: q of the previous plane (two register sets that swap roles in
+  // the x loop unrolled by two, so the rotation costs no moves) and A = P + f of it
+  Vec<T> QA[GW], QB[GW], CA[GW];
+  Vec<T> UA, UB;  // 2cx u of the previous plane (the face between it and the arriving one): swap like q
+#pragma unroll
+  for (int e = 0; e < NK; ++e) UA.v[e] = T(0);
+#pragma unroll
+  for (int s = 0; s < GW; ++s) {
+#pragma unroll
+    for (int e = 0; e < NK; ++e) QA[s].v[e] = CA[s].v[e] = T(0);
+  }
+  int st = 0;
+  uint32_t par = 0, pA = a0;
+  long long c = c0;
+
+  auto step = [&](auto store_tag, const Vec<T> (&QP)[GW], Vec<T> (&QN)[GW], const Vec<T> &ux, Vec<T> &un) {
+    constexpr bool STORE = decltype(store_tag)::value;
+    mbar_wait(bar0 + 8 * st, par);  // the next plane has landed
+    const uint32_t pV = pA + fb, pW = pV + fb;
+    Vec<T> vs = lds_at<-RSB>(pV, tag), vn = lds_at<0>(pV, tag);
+    Vec<T> wt = lds_at<0>(pW, tag);
+    Vec<T> wl = down_with(wt, lds1_at<-SZ>(pW, tag));  // w one level below each element
+    un = lds_at<0>(pA, tag);  // read now: the slot's release must not wait for it
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      vs.v[e] *= cy2; vn.v[e] *= cy2;
+      wl.v[e] *= c1.v[e]; wt.v[e] *= c2.v[e];
+      un.v[e] *= cx2;
+    }
+    uint32_t pQ = pA + q0off;
+#pragma unroll
+    for (int s = 0; s < GW; ++s) {
+      if (FULL || s < mycnt) {  // warp-uniform
+        QN[s] = lds_at<0>(pQ, tag);
+        const Vec<T> &q = QN[s];
+        const Vec<T> qS = lds_at<-RSB>(pQ, tag), qN = lds_at<RSB>(pQ, tag);
+        const Vec<T> qU = up_with(q, lds1_at<UP>(pQ, tag));
+        // the level below the thread's first: lane 0 reads it, the others get it by shuffle
+        const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
+        Vec<T> o;
+        if (SKEW) {
+          // Piacsek-Williams skew form (R4): the advected parenthesis holds the
+          // far value only, so each face contributes the neighbour's value times the
+          // (scaled) advecting velocity
+          const T prv = __shfl_up_sync(kFull, q.v[NK - 1], 1);
+          const Vec<T> qD = down_with(q, lane == 0 ? qb : prv);
+#pragma unroll
+          for (int e = 0; e < NK; ++e) {
+            T y = vn.v[e] * qN.v[e];
+            y = vs.v[e] * qS.v[e] - y;
+            y = wl.v[e] * qD.v[e] + y;
+            y = y - wt.v[e] * qU.v[e];
+            o.v[e] = CA[s].v[e] - ux.v[e] * q.v[e];
+            CA[s].v[e] = y + ux.v[e] * QP[s].v[e];
+          }
+        } else {
+          Vec<T> g;
+#pragma unroll
+          for (int e = 0; e < NK; ++e) g.v[e] = q.v[e] + qU.v[e];
+          const T prv = __shfl_up_sync(kFull, g.v[NK - 1], 1);
+          const Vec<T> gD = down_with(g, lane == 0 ? qb + q.v[0] : prv);
+#pragma unroll
+          for (int e = 0; e < NK; ++e) {
+            T y = vn.v[e] * (q.v[e] + qN.v[e]);
+            y = vs.v[e] * (qS.v[e] + q.v[e]) - y;
+            y = wl.v[e] * gD.v[e] + y;
+            y = y - wt.v[e] * g.v[e];  // P: the y and z flux differences of this plane
+            const T sx = QP[s].v[e] + q.v[e];
+            o.v[e] = CA[s].v[e] - ux.v[e] * sx;  // minus the flux through the face between the two planes
+            CA[s].v[e] = y + ux.v[e] * sx;
+          }
+        }
+        if (STORE && act) {  // sq of the previous plane is complete
+          o.v[0] = keep_if(o.v[0], keep_first);
+          T *sq = sqp[s] + c;  // pointer table lives in the constant bank
+          if (ACC) {
+            const Vec<T> a = ld_vec_rw(sq);
+#pragma unroll
+            for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
+          }
+          st_vec(sq, o);
+        }
+        pQ += fb;
+      }
+    }
+    // this warp is done with the slot
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
+    if (STORE) c += plane;
+    pA += sbytes;
+    if (++st == nstages) { st = 0; par ^= 1; pA = a0; }
+  };
+  // plane i0-1 only leaves q and u behind, plane i0 the first A; from then on every
+  // plane completes the tendencies of the one before it
+  step(std::false_type{}, QA, QB, UA, UB);
+  step(std::false_type{}, QB, QA, UB, UA);
+  int left = nplanes - 2;
+#pragma unroll 1
+  while (left > 0) {
+    step(std::true_type{}, QA, QB, UA, UB);
+    if (--left == 0) break;
+    step(std::true_type{}, QB, QA, UB, UA);
+    --left;
+  }
+}
 
 template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const MomPtrs<T> mo, const int nq, const int ngroups, const int gb, const int ty,
-            const int zw, const int ss, const int nstages, const int fieldsz) {
+            const int ss, const int nstages, const int fieldsz) {
   constexpr int NK = VecOf<T>::NK;
+  constexpr int SZ = (int)sizeof(T);
+  constexpr int ZB = 32 * NK;                // levels per block tile
+  constexpr int RS = kRowBytes / SZ;         // row stride in elements
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int ZB = zw * 32 * NK;   // levels per block tile
-  const int RS = ZB + 2 * NK;    // row stride: one 16-byte vector of z halo on each side
   const int rows = ty + 2;
   const int stagesz = (3 + gb) * fieldsz;
-  T *tiles = reinterpret_cast<T *>(smem_raw);
-  const uint32_t bar0 = smem_u32(smem_raw + (size_t)nstages * stagesz * sizeof(T));
+  const uint32_t t0 = smem_u32(smem_raw);
+  const uint32_t bar0 = t0 + (uint32_t)(nstages * stagesz * SZ);
   // full[s] at bar0 + 8 s, empty[s] at bar0 + 8 (nstages + s)
 
   // block -> (scalar group, z tile, y tile); group fastest so that the blocks
@@ -510,14 +681,13 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   const int jr0 = yt * ty;
   const int ncol = min(ty, p.ny - jr0);
   const int kb0 = zt * ZB;
-  const int zlive = min(zw, (nz - kb0 + 32 * NK - 1) / (32 * NK));  // z chunks with a level < nz
-  const int slive = (cnt + GW - 1) / GW;                             // splits with a scalar
-  const int nr = ss + (MOM ? 1 : 0);                                 // roles per column chunk
-  const int ncw = ncol * zlive * (slive + (MOM ? 1 : 0));            // live consumer warps
+  const int slive = (cnt + GW - 1) / GW;                   // splits with a scalar
+  const int nr = ss + (MOM ? 1 : 0);                       // roles per column
+  const int ncw = ncol * (slive + (MOM ? 1 : 0));          // live consumer warps
   const int i0 = p.ia + blockIdx.y * p.xc;
   const int i1 = min(p.ib, i0 + p.xc);
   const int nplanes = i1 - i0 + 2;  // planes i0-1 .. i1
-  const int nwarps_c = ty * zw * nr;
+  const int nwarps_c = ty * nr;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < nstages; ++s) {
@@ -532,11 +702,11 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   if (warp == nwarps_c) {
     // ---------------- producer warp: one lane per field ----------------
     const int nfld = 3 + cnt;
-    const uint32_t box_bytes = (uint32_t)(rows * RS * (int)sizeof(T));
+    const uint32_t box_bytes = (uint32_t)(rows * kRowBytes);
     const CUtensorMap *mymap = &maps.m[lane < 3 ? lane : 3 + s0 + min(lane - 3, cnt - 1)];
     if (lane < nfld) prefetch_tensormap(mymap);
     pdl_wait();  // the fields may have been written by the previous kernel in the stream
-    const uint32_t t0 = smem_u32(tiles);
+    const uint32_t dst0 = t0 + (uint32_t)(lane * fieldsz * SZ);
     int s = 0;
     uint32_t par = 1;  // a fresh mbarrier passes a wait on parity 1: the first lap does not block
 #pragma unroll 1
@@ -546,105 +716,41 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
       if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
       __syncwarp();
       if (lane < nfld)
-        tma_load_3d(t0 + (uint32_t)((s * stagesz + lane * fieldsz) * (int)sizeof(T)), mymap,
-                    kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+        tma_load_3d(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
       if (++s == nstages) { s = 0; par ^= 1; }
     }
     return;
   }
 
   // ---------------- consumers ----------------
-  const int col = warp / (zw * nr);
-  const int rem = warp - col * (zw * nr);
-  const int zc = rem / nr;
-  const int sp = rem - zc * nr;
-  if (col >= ncol || zc >= zlive) return;
-  const int k0r = kb0 + (zc * 32 + lane) * NK;
+  const int col = warp / nr;
+  const int sp = warp - col * nr;
+  if (col >= ncol) return;
+  const int k0r = kb0 + lane * NK;
   const bool act = k0r < nz;
   const int k0 = act ? k0r : nz - NK;  // clamp: finite data, never stored
   const bool bot_edge = act && lane == 0 && k0 > 0;
-  const int e0 = (col + 1) * RS + (k0 - (kb0 - NK));  // element index inside a field tile
+  const uint32_t fb = (uint32_t)(fieldsz * SZ), sbytes = (uint32_t)(stagesz * SZ);
+  // u(column, k0) in stage 0: row col+1 of the box, one vector of z halo before level kb0
+  const uint32_t a0 = t0 + (uint32_t)(((col + 1) * RS + (k0 - kb0 + NK)) * SZ);
+  const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+  const int keep_first = k0 == 0 ? 0 : -1;  // element 0 is level K = 1: no tendency
   if (MOM && sp == ss) {
     // ---------------- momentum role (fused launch): su, sv, sw of this column chunk
-    // from the wind tiles the scalar warps use.  Same x march as tma_momentum; a
-    // plane is read when it lands (as the east plane) and once more one step
-    // later (as the centre plane), so its slot is released one step late.
-    constexpr int SZm = (int)sizeof(T);
-    constexpr int UPm = NK * SZm;
-    const T *const tg = nullptr;
-    const Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
-    const Vec<T> d1 = ld_vec(p.tzd1 + k0), d2 = ld_vec(p.tzd2 + k0);
-    const T cx = p.cx, cy = p.cy;
-    const bool first_level = k0 == 0, last_level = k0 + NK == nz;
-    const uint32_t fb = (uint32_t)(fieldsz * SZm), sbytes = (uint32_t)(stagesz * SZm);
-    const uint32_t rsb = (uint32_t)(RS * SZm);
-    const uint32_t a0 = smem_u32(tiles) + (uint32_t)(e0 * SZm);  // u(column, k0) in stage 0
-    const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
-    T *qu = mo.su + c0, *qv = mo.sv + c0, *qw = mo.sw + c0;
-    const long long plane = p.plane;
+    // from the wind tiles the scalar warps use
+    MarchArgs<T> m;
+    m.c1 = ld_vec(p.tzc1 + k0); m.c2 = ld_vec(p.tzc2 + k0);
+    m.d1 = ld_vec(p.tzd1 + k0); m.d2 = ld_vec(p.tzd2 + k0);
+    m.a0 = a0; m.fb = fb; m.sbytes = sbytes; m.rsb = (uint32_t)kRowBytes; m.bar0 = bar0;
+    m.nstages = nstages; m.nsteps = nplanes - 1; m.lane = lane;
+    m.act = act; m.bot_edge = bot_edge;
+    m.first_level = k0 == 0;
+    m.last_level = k0 + NK == nz;
+    m.su = mo.su; m.sv = mo.sv; m.sw = mo.sw;
+    m.c0 = c0; m.plane = p.plane;
+    m.cx = p.cx; m.cy = p.cy;
     pdl_wait();
-    mbar_wait(bar0, 0);  // plane i0-1
-    PlaneRegs<T> RA, RB;
-    XFlux<T> FA, FB;
-    RA.u = lds_at<0>(a0, tg);
-    RA.v = lds_at<0>(a0 + fb, tg);
-    RA.vs = lds_at<0>(a0 + fb - rsb, tg);
-    RA.w = lds_at<0>(a0 + 2 * fb, tg);
-#pragma unroll
-    for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
-    int sC = 0, sE = 1 % nstages, t = 0;
-    uint32_t parE = (nstages == 1) ? 1 : 0;
-    uint32_t pC = a0, pE = a0 + (uint32_t)sE * sbytes;
-    const int nsteps = nplanes - 1;
-    auto mstep = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
-      mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
-      const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
-      const Vec<T> uS = lds_at<0>(pC - rsb, tg), uN = lds_at<0>(pC + rsb, tg);
-      const Vec<T> vN = lds_at<0>(pCv + rsb, tg);
-      const Vec<T> wS = lds_at<0>(pCw - rsb, tg), wN = lds_at<0>(pCw + rsb, tg);
-      RE.u = lds_at<0>(pE, tg);
-      RE.v = lds_at<0>(pEv, tg);
-      RE.vs = lds_at<0>(pEv - rsb, tg);
-      RE.w = lds_at<0>(pEv + fb, tg);
-      const Vec<T> uCu = up_with(RC.u, lds1_at<UPm>(pC, tg)), vCu = up_with(RC.v, lds1_at<UPm>(pCv, tg));
-      const Vec<T> wCu = up_with(RC.w, lds1_at<UPm>(pCw, tg));
-      const Vec<T> vSu = up_with(RC.vs, lds1_at<UPm>(pCv - rsb, tg));
-      BelowEdge<T> be;
-      if (bot_edge) {
-        be.ub = lds1_at<-SZm>(pC, tg); be.vb = lds1_at<-SZm>(pCv, tg); be.wb = lds1_at<-SZm>(pCw, tg);
-        be.web = lds1_at<-SZm>(pEv + fb, tg); be.wnb = lds1_at<-SZm>(pCw + rsb, tg);
-      }
-      Vec<T> ou, ov, ow;
-      momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, bot_edge, be, c1,
-                              c2, d1, d2, cx, cy, lane, ou, ov, ow);
-      if (first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
-      if (last_level) ow.v[NK - 1] = T(0);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));  // done with the centre plane's slot
-      if (t > 0) {
-        if (act) {
-          if (ACC) {
-            const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
-#pragma unroll
-            for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
-          }
-          st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
-        }
-        qu += plane; qv += plane; qw += plane;
-      }
-      sC = sE;
-      pC = pE;
-      pE += sbytes;
-      if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
-      ++t;
-    };
-#pragma unroll 1
-    while (true) {
-      mstep(RA, RB, FA, FB);
-      if (t == nsteps) break;
-      mstep(RB, RA, FB, FA);
-      if (t == nsteps) break;
-    }
+    momentum_march<T, ACC, SKEW>(m, []() {});
     return;
   }
   if (sp >= slive) return;
@@ -654,106 +760,15 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
 #pragma unroll
   for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
   const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
-  long long c = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
+  const uint32_t q0off = (uint32_t)(3 + sb) * fb;  // this warp's first scalar
+  T *const *sqp = outs.sq + (s0 + sb);
   pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
-
-  // carried from the previous plane, per scalar: q, the x flux through its west
-  // face and the y + z part of its tendency.  (Swapping two register sets in an
-  // x loop unrolled by two, as tma_momentum does, spills here: measured slower.)
-  struct Carry { Vec<T> q, fx, P; };
-  Carry CA[GW], CB[GW];
-  Vec<T> uA, uB;
-#pragma unroll
-  for (int e = 0; e < NK; ++e) uA.v[e] = T(0);
-#pragma unroll
-  for (int s = 0; s < GW; ++s) {
-#pragma unroll
-    for (int e = 0; e < NK; ++e) CA[s].q.v[e] = CA[s].fx.v[e] = CA[s].P.v[e] = T(0);
-  }
-  constexpr int SZ = (int)sizeof(T);
-  constexpr int UP = NK * SZ;
-  const T *const tag = nullptr;
-  const bool first_level = k0 == 0;  // element 0 is level K = 1: no tendency
-  const uint32_t fb = (uint32_t)(fieldsz * SZ), sbytes = (uint32_t)(stagesz * SZ), rsb = (uint32_t)(RS * SZ);
-  const uint32_t a0 = smem_u32(tiles) + (uint32_t)(e0 * SZ);   // u(column, k0) in stage 0
-  const uint32_t q0off = (uint32_t)(3 + sb) * fb;              // this warp's first scalar
-  const long long plane = p.plane;
-
-  int st = 0, t = 0;
-  uint32_t par = 0;
-  uint32_t pA = a0;
-  auto step = [&](const Carry (&CP)[GW], Carry (&CN)[GW], const Vec<T> &uP, Vec<T> &uN) {
-    mbar_wait(bar0 + 8 * st, par);  // plane i0-1+t has landed
-    const uint32_t pV = pA + fb, pW = pV + fb;
-    uN = lds_at<0>(pA, tag);
-    const Vec<T> vC = lds_at<0>(pV, tag), vS = lds_at<0>(pV - rsb, tag), wC = lds_at<0>(pW, tag);
-    const T wb = bot_edge ? lds1_at<-SZ>(pW, tag) : T(0);
-    const bool store = act && t >= 2;
-    uint32_t pQ = pA + q0off;
-#pragma unroll
-    for (int s = 0; s < GW; ++s) {
-      if (s < mycnt) {  // warp-uniform
-        const Vec<T> q = lds_at<0>(pQ, tag);
-        const Vec<T> qS = lds_at<0>(pQ - rsb, tag), qN = lds_at<0>(pQ + rsb, tag);
-        const Vec<T> qU = up_with(q, lds1_at<UP>(pQ, tag));
-        // SKEW (Piacsek-Williams skew form, R4): the advected parenthesis
-        // holds the far value only, so a face carries two products: the one of
-        // the point across the face is handed on (fx in x, the shuffle in z).
-        const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
-        const T b_z = SKEW ? wb * qb : wb * (qb + q.v[0]);
-        Vec<T> fz_t, fz_p, hy, fx_e;
-#pragma unroll
-        for (int e = 0; e < NK; ++e) {
-          if (SKEW) {
-            fx_e.v[e] = uP.v[e] * q.v[e];            // east face of plane i-1, seen from i-1
-            CN[s].fx.v[e] = uP.v[e] * CP[s].q.v[e];  // the same face seen from plane i
-            hy.v[e] = cy2 * (vS.v[e] * qS.v[e] - vC.v[e] * qN.v[e]);
-            fz_t.v[e] = wC.v[e] * qU.v[e];
-            fz_p.v[e] = wC.v[e] * q.v[e];
-          } else {
-            CN[s].fx.v[e] = uP.v[e] * (CP[s].q.v[e] + q.v[e]);  // face between planes i-1 and i
-            fx_e.v[e] = CN[s].fx.v[e];
-            hy.v[e] = cy2 * (vS.v[e] * (qS.v[e] + q.v[e]) - vC.v[e] * (q.v[e] + qN.v[e]));
-            fz_t.v[e] = wC.v[e] * (q.v[e] + qU.v[e]);
-            fz_p.v[e] = fz_t.v[e];
-          }
-        }
-        const Vec<T> fz_b = shift_down(fz_p, lane, b_z);
-        if (store) {  // sq of plane i-1 is complete
-          Vec<T> o;
-#pragma unroll
-          for (int e = 0; e < NK; ++e) o.v[e] = CP[s].P.v[e] + cx2 * (CP[s].fx.v[e] - fx_e.v[e]);
-          if (first_level) o.v[0] = T(0);
-          T *sq = outs.sq[s0 + sb + s] + c;  // pointer table lives in the constant bank
-          if (ACC) {
-            const Vec<T> a = ld_vec_rw(sq);
-#pragma unroll
-            for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
-          }
-          st_vec(sq, o);
-        }
-#pragma unroll
-        for (int e = 0; e < NK; ++e)
-          CN[s].P.v[e] = hy.v[e] + (c1.v[e] * fz_b.v[e] - c2.v[e] * fz_t.v[e]);
-        CN[s].q = q;
-        pQ += fb;
-      }
-    }
-    // this warp is done with the slot
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
-    if (t >= 2) c += plane;
-    pA += sbytes;
-    if (++st == nstages) { st = 0; par ^= 1; pA = a0; }
-    ++t;
-  };
-#pragma unroll 1
-  while (t < nplanes) {
-    step(CA, CB, uA, uB);
-    uA = uB;
-#pragma unroll
-    for (int s = 0; s < GW; ++s) CA[s] = CB[s];
-  }
+  if (mycnt == GW)
+    scalar_march<T, GW, ACC, SKEW, true>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, lane, act,
+                                         bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+  else
+    scalar_march<T, GW, ACC, SKEW, false>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, lane, act,
+                                          bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
 }
 
 }  // namespace monc
