@@ -27,8 +27,9 @@
  *   - Halo entries of output arrays are never written.
  *   - Inputs need valid halos to depth 1 in x and y (the library does no halo
  *     exchange: PAPER.md:49 does it in an earlier timestep group).
- *   - Inputs and outputs must not alias.  All base pointers must be 16-byte
- *     aligned.
+ *   - No output array may overlap an input array or another output array
+ *     (checked over the whole arrays, not only the base pointers: EINVAL).  All
+ *     base pointers must be 16-byte aligned.
  *   - Every call returns MONC_ADV_OK (0) or a negative error code, never
  *     throws or aborts; monc_adv_last_error gives the text of the last
  *     failure on that handle.
@@ -133,14 +134,25 @@ int monc_adv_tendencies(monc_adv_t h, const void *u, const void *v, const void *
  * and shared by the momentum and scalar kernels.
  *   hu, hv, hw, hq[n]: pinned host inputs, E elements each, valid halos.
  *   hsu, hsv, hsw, hsq[n]: pinned host outputs; only INTERIOR entries are
- *     written (the GPU result lands in this separate buffer; the host adds it
- *     to its own source terms).  hsu/hsv/hsw may ALL be NULL
- *     to advect scalars only.
+ *     written.  Default (overwrite): the GPU result lands in this separate
+ *     buffer and the host adds it to its own source terms.
+ *     With monc_adv_set_accumulate(h, 1) the arrays are IN/OUT: they hold the
+ *     host's own source terms, each chunk's slab of them is uploaded with the
+ *     fields, the kernels add the advection tendencies on the device
+ *      and the combined source terms come back into the same
+ *     arrays -- bitwise equal to waiting for the step and adding on the host,
+ *     without the extra result buffer PAPER.md:99 needs.  hsu/hsv/hsw may ALL be
+ *     NULL to advect scalars only.
  *   hq, hsq: host arrays of nq host pointers (may be NULL when nq = 0).
  *   cuda_stream: work already queued on it is waited for before the first
  *     copy; NULL = no dependency.
  * Device staging buffers (3+nq inputs, 3+nq outputs) are allocated on first
- * use and reused.  Errors: EBUSY if the previous step was not waited for.
+ * use and reused.  Errors: EBUSY if the previous step was not waited for;
+ * EINVAL if an array is not page-locked over its whole length (pageable memory
+ * would silently turn the asynchronous copies into synchronous ones, the very
+ * failure PAPER.md:95 describes) or if arrays overlap.  If a CUDA call fails
+ * part-way through the enqueue, what was queued is waited for, the error is
+ * returned and no step is in flight: the handle stays usable.
  */
 int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void *hw,
                         const void *const *hq, int nq, void *hsu, void *hsv, void *hsw,
@@ -149,8 +161,10 @@ int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void
 /* Block until every H2D copy of the in-flight step is done: the host may then
  * overwrite its input fields. */
 int monc_adv_step_inputs_consumed(monc_adv_t h);
-/* Block until chunk c's tendencies are in host memory (enables the streaming
- * combine PAPER.md:101 wishes for).  0 <= c < nchunks. */
+/* Block until chunk c's tendencies are in host memory: the host can integrate
+ * the source terms of that slab while the later chunks are still streaming back
+ * ("overlapping computation with data copying, rather than waiting for the entire
+ * data copy").  0 <= c < nchunks. */
 int monc_adv_step_wait_chunk(monc_adv_t h, int c);
 /* Block until all tendencies of the in-flight step are in host memory and
  * mark the step complete.  No-op if no step is in flight. */
@@ -174,36 +188,12 @@ int monc_adv_set_overlap(monc_adv_t h, int on);
  * dropped from every advected-quantity parenthesis).  Both forms run on the
  * generic kernels and on the TMA kernels (variants 1 and 3). */
 int monc_adv_set_form(monc_adv_t h, int form);
-/* 0 (default): tendencies overwritten.  1: added into the output buffers. */
+/* 0 (default): tendencies overwritten.  1: added into the output buffers (device
+ * arrays of momentum / scalars / tendencies; host arrays of step_async, see there). */
 int monc_adv_set_accumulate(monc_adv_t h, int on);
-/* 1 (default): the TMA kernels are launched with CUDA's programmatic
- * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
- * predecessor in the stream (it waits for the predecessor's completion before
- * touching any field: results are unchanged).  0: plain stream order. */
-int monc_adv_set_pdl(monc_adv_t h, int on);
 /* 1 (default): monc_adv_tendencies and monc_adv_step_async use the fused
  * momentum + scalars launch where it fits.  0: always two launches. */
 int monc_adv_set_fuse(monc_adv_t h, int on);
-/* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
- * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
- * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need
- * nz % (16/sizeof(dtype)) == 0; 2 also needs the flux form. */
-int monc_adv_set_variant(monc_adv_t h, int variant);
-/* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
- * that makes sense.
- *   xchunk:   planes marched by one thread block;
- *   group:    scalars that share one staged copy of the wind: per thread block
- *             (1..10) in variant 3, per thread (1..5) in variant 2;
- *   prefetch: L2 prefetch distance in planes (-1 = no prefetch), variant 2;
- *   warps:    variant 2: warps per thread block (1..8); ignored by variant 3 (a
- *             block tile is one 32-vector z chunk per column);
- *   stages:   depth of the TMA ring (2..8), variant 3;
- *   tile_y:   columns per thread block, variant 3;
- *   split:    variant 3 scalars: warps that share one column chunk and split
- *             the block's scalars between them (1..4). */
-int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
-                        int tile_y, int split);
-
 /* Copy the coefficient tables the handle uses to HOST arrays of nz doubles
  * (as stored, i.e. after rounding to fp32 for an F32 handle).  Any pointer
  * may be NULL. */

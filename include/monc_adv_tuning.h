@@ -1,0 +1,45 @@
+/*
+ * monc_adv_tuning.h -- INTERNAL knobs of libmonc_adv.so: kernel family, launch
+ * geometry, launch attribute.  For the library's own tests, benchmarks and
+ * profiling; not part of the interface a model links against (include/monc_adv.h)
+ * and free to change.  The defaults (0 everywhere) are what the library's launch
+ * planners choose; results do not depend on any of these.
+ */
+#ifndef MONC_ADV_TUNING_H
+#define MONC_ADV_TUNING_H
+
+#include "monc_adv.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
+ * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
+ * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need
+ * nz % (16/sizeof(dtype)) == 0; 2 also needs the flux form. */
+int monc_adv_set_variant(monc_adv_t h, int variant);
+/* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
+ * that makes sense.
+ *   xchunk:   planes marched by one thread block;
+ *   group:    scalars that share one staged copy of the wind: per thread block
+ *             (1..10) in variant 3, per thread (1..5) in variant 2;
+ *   prefetch: L2 prefetch distance in planes (-1 = no prefetch), variant 2;
+ *   warps:    variant 2: warps per thread block (1..8); ignored by variant 3 (a
+ *             block tile is one 32-vector z chunk per column);
+ *   stages:   depth of the TMA ring (2..8), variant 3;
+ *   tile_y:   columns per thread block, variant 3;
+ *   split:    variant 3 scalars: warps that share one column chunk and split
+ *             the block's scalars between them (1..4). */
+int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
+                        int tile_y, int split);
+
+/* 1 (default): the TMA kernels are launched with CUDA's programmatic
+ * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
+ * predecessor in the stream (it waits for the predecessor's completion before
+ * touching any field: results are unchanged).  0: plain stream order. */
+int monc_adv_set_pdl(monc_adv_t h, int on);
+#ifdef __cplusplus
+}
+#endif
+#endif /* MONC_ADV_TUNING_H */

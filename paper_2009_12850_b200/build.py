@@ -16,7 +16,8 @@ LIB = os.path.join(HERE, "libmonc_adv.so")
 SOURCES = [os.path.join(CSRC, "monc_adv.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "monc_adv_kernels.cuh"),
                   os.path.join(CSRC, "monc_adv_tma.cuh"),
-                  os.path.join(ROOT, "include", "monc_adv.h")]
+                  os.path.join(ROOT, "include", "monc_adv.h"),
+                  os.path.join(ROOT, "include", "monc_adv_tuning.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",

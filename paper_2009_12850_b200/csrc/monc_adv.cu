@@ -5,6 +5,7 @@
 // 99-101): chunked H2D -> kernels -> D2H on separate streams with events.
 // No torch types, no CPU compute fallback: if CUDA fails the call fails.
 #include "monc_adv.h"
+#include "monc_adv_tuning.h"
 #include "monc_adv_kernels.cuh"
 #include "monc_adv_tma.cuh"
 
@@ -13,8 +14,13 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <set>
 #include <string>
+#include <tuple>
+#include <utility>
 #include <vector>
 
 using namespace monc;
@@ -22,6 +28,29 @@ using namespace monc;
 namespace {
 thread_local std::string g_create_error;
 }
+
+// geometry of the TMA-staged kernels: TY columns per block, ring depth S
+struct TmaPlan {
+  bool ok = false;
+  int ty = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0;
+  size_t smem = 0;
+};
+// geometry of tma_scalars: ty columns x ss scalar splits = consumer warps per
+// block; gb scalars per block (gw per warp); ring depth S.  A stage holds 3 + gb
+// field tiles of (ty+2) rows of kRowBytes (each tile rounded up to 128 B).
+struct TmaScalarPlan {
+  bool ok = false;
+  int ty = 0, ss = 0, gb = 0, gw = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0, fieldsz = 0;
+  size_t smem = 0;
+};
+// tensor-map descriptors of one launch, kept while the same arrays come back
+// (the chunks of a hybrid step, the rotating buffer sets of a time loop)
+struct MapEntry {
+  std::vector<const void *> ptrs;  // u, v, w, q[0..n)
+  int ty = 0;
+  unsigned long stamp = 0;
+  TensorMaps maps;
+};
 
 struct monc_adv_s {
   int nx = 0, ny = 0, nz = 0, h = 0, dtype = 0;
@@ -40,6 +69,11 @@ struct monc_adv_s {
   long launches = 0;
   std::string err;
   std::string plan_mom, plan_sca, plan_text;  // geometry of the last launches
+  // launch plans by (planes, scalars, fused); dropped when a tuning knob changes
+  std::map<int, TmaPlan> mom_plans;
+  std::map<std::tuple<int, int, int>, TmaScalarPlan> sca_plans;
+  std::vector<MapEntry> map_cache;
+  unsigned long map_clock = 0;
   // ---- async step state
   int nchunks = 8, overlap = 1;
   int staged_nq = -1;
@@ -69,6 +103,38 @@ int cuda_fail(monc_adv_t h, cudaError_t e, const char *what) {
   } while (0)
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// two arrays of `bytes` bytes each share at least one byte
+bool ranges_overlap(const void *a, const void *b, size_t bytes) {
+  const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+  return x < y ? y - x < bytes : x - y < bytes;
+}
+// first (input, output) or (output, output) pair of whole-field arrays that overlap
+const char *find_alias(const std::vector<const void *> &ins, const std::vector<const void *> &outs,
+                       size_t bytes) {
+  for (size_t b = 0; b < outs.size(); ++b) {
+    for (const void *a : ins)
+      if (ranges_overlap(a, outs[b], bytes)) return "inputs and outputs must not overlap";
+    for (size_t c = 0; c < b; ++c)
+      if (ranges_overlap(outs[c], outs[b], bytes)) return "outputs must not overlap each other";
+  }
+  return nullptr;
+}
+// host memory the copy engines can read asynchronously: page-locked (cudaMallocHost,
+// cudaHostRegister) or managed, over the whole array.  Pageable memory would make
+// every "asynchronous" copy a synchronous staged one -- the silent fallback PAPER.md:95
+// ran into -- so it is refused.
+bool is_pinned_host(const void *p, size_t bytes) {
+  for (const char *q : {(const char *)p, (const char *)p + bytes - 1}) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, q) != cudaSuccess) {
+      cudaGetLastError();
+      return false;
+    }
+    if (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged) return false;
+  }
+  return true;
+}
 
 template <typename T>
 KParams<T> make_params(monc_adv_t h, int ia, int ib) {
@@ -131,15 +197,8 @@ double launch_rounds(long blocks, int sm_count) {
   return 1.12 * (double)blocks / (double)sm_count + 0.5;
 }
 
-// geometry of the TMA-staged kernels: TY columns per block, ring depth S
-struct TmaPlan {
-  bool ok = false;
-  int ty = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0;
-  size_t smem = 0;
-};
-
 template <typename T>
-TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
+TmaPlan compute_plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
   TmaPlan pl;
   constexpr int NK = VecOf<T>::NK;
   if (h->nz % NK != 0) return pl;
@@ -179,6 +238,30 @@ TmaPlan plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
   return pl;
 }
 
+// plans depend on the handle's sizes and tuning knobs and on the call's plane
+// count only: computed once, kept on the handle (dropped by set_tuning)
+template <typename T>
+const TmaPlan &plan_tma(monc_adv_t h, int nplanes) {
+  auto it = h->mom_plans.find(nplanes);
+  if (it == h->mom_plans.end()) it = h->mom_plans.emplace(nplanes, compute_plan_tma<T>(h, nplanes, 3)).first;
+  return it->second;
+}
+
+// The dynamic shared-memory limit of a kernel is raised ONCE per device to the
+// opt-in maximum (the attribute is per context: setting the exact size of each
+// plan before each launch would let two handles lower each other's limit).
+template <typename K>
+cudaError_t allow_max_smem(monc_adv_t h, K kernel) {
+  static std::mutex mu;
+  static std::set<std::pair<int, const void *>> done;
+  std::lock_guard<std::mutex> lock(mu);
+  const auto key = std::make_pair(h->device, reinterpret_cast<const void *>(kernel));
+  if (done.count(key)) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin);
+  if (e == cudaSuccess) done.insert(key);
+  return e;
+}
+
 // Launch with the programmatic stream-serialisation attribute (PDL): the kernel
 // may begin (barrier set-up, coefficient loads) while its predecessor in the
 // stream drains; it calls griddepcontrol.wait before touching any field.
@@ -204,14 +287,14 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
   if (ib <= ia) return MONC_ADV_OK;
   KParams<T> p = make_params<T>(h, ia, ib);
   TmaPlan pl;
-  if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia, 3);
+  if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia);
   if (h->variant == 3 && !pl.ok)
     return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
   if (pl.ok) {
     p.xc = pl.xc;
     dim3 grid(pl.tiles, pl.nchunks);
     auto go = [&](auto kernel) -> int {
-      CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+      CU(allow_max_smem(h, kernel));
       CU(launch_pdl(h, kernel, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages, u, v, w, su, sv, sw));
       return MONC_ADV_OK;
     };
@@ -279,23 +362,12 @@ bool encode_field_map(monc_adv_t h, CUtensorMap *m, const void *base, int box_z,
              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// geometry of tma_scalars: ty columns x zw z-chunks (32 vectors each) x ss
-// scalar splits = consumer warps per block; gb scalars per block (gw per
-// warp); ring depth S.  A stage holds 3 + gb field tiles of (ty+2) rows of
-// ZB + 2*NK elements (each tile rounded up to 128 B).
-struct TmaScalarPlan {
-  bool ok = false;
-  int ty = 0, zw = 0, ss = 0, gb = 0, gw = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0, fieldsz = 0;
-  size_t smem = 0;
-};
-
 template <typename T>
-TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = false) {
+TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom) {
   TmaScalarPlan pl;
   constexpr int NK = VecOf<T>::NK;
   if (h->nz % NK != 0 || !tensor_map_encoder()) return pl;
   const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
-  const int wzc = (h->nz / NK + 31) / 32;  // warps a whole column needs
   const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
   double best = 1e300;
   // Cost model, calibrated on B200:
@@ -314,10 +386,10 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
       const int gw = (gb + ss - 1) / ss;
       if (gw > 5) continue;
       {
-        constexpr int zw = 1;  // one 32-vector z chunk per block tile: the row stride is a compile-time constant
+        // one 32-vector z chunk per block tile: the row stride is a compile-time constant
         const int ZB = 32 * NK, RS = kRowBytes / (int)sizeof(T);
         const int nzt = (h->nz + ZB - 1) / ZB;
-        const int tymax = std::min(h->ny, kScalarConsumerWarps / (zw * (ss + (mom ? 1 : 0))));
+        const int tymax = std::min(h->ny, kScalarConsumerWarps / (ss + (mom ? 1 : 0)));
         if (tymax < 1) continue;
         for (int ty = tymax; ty >= 1; --ty) {
           if (h->tile_y > 0 && ty != std::min(h->tile_y, tymax)) continue;
@@ -348,7 +420,7 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
             const double cost = waves * (xc + (waves <= 1.3 ? 4 : 3)) * t_step * march;
             if (cost < best) {
               best = cost;
-              pl.ok = true; pl.ty = ty; pl.zw = zw; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
+              pl.ok = true; pl.ty = ty; pl.ss = ss; pl.gb = gb; pl.gw = gw; pl.stages = S;
               pl.xc = xc; pl.tiles = tiles;
               pl.nchunks = (nplanes + xc - 1) / xc;
               pl.fieldsz = (int)(field / sizeof(T));
@@ -362,13 +434,62 @@ TmaScalarPlan plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom = fals
   return pl;
 }
 
+template <typename T>
+const TmaScalarPlan &plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom) {
+  const auto key = std::make_tuple(nplanes, n, mom ? 1 : 0);
+  auto it = h->sca_plans.find(key);
+  if (it == h->sca_plans.end())
+    it = h->sca_plans.emplace(key, compute_plan_tma_scalars<T>(h, nplanes, n, mom)).first;
+  return it->second;
+}
+
+// Tensor-map descriptors for (u, v, w, q[0..n)) with ty+2 rows per box: encoded
+// when first seen, then reused (at most kMapCacheEntries sets, least recently
+// used replaced).  Unused slots of the launch repeat the first scalar.
+constexpr size_t kMapCacheEntries = 8;
+template <typename T>
+const TensorMaps *field_maps(monc_adv_t h, const T *u, const T *v, const T *w, const void *const *q, int n,
+                             int ty) {
+  std::vector<const void *> ptrs = {u, v, w};
+  for (int s = 0; s < n; ++s) ptrs.push_back(q[s]);
+  for (MapEntry &e : h->map_cache)
+    if (e.ty == ty && e.ptrs == ptrs) {
+      e.stamp = ++h->map_clock;
+      return &e.maps;
+    }
+  MapEntry *slot = nullptr;
+  if (h->map_cache.size() < kMapCacheEntries) {
+    h->map_cache.reserve(kMapCacheEntries);
+    h->map_cache.emplace_back();
+    slot = &h->map_cache.back();
+  } else {
+    slot = &h->map_cache[0];
+    for (MapEntry &e : h->map_cache)
+      if (e.stamp < slot->stamp) slot = &e;
+  }
+  const int RS = kRowBytes / (int)sizeof(T);
+  bool ok = true;
+  for (int f = 0; f < 3 + kMaxScalarsPerLaunch; ++f) {
+    const void *base = f < 3 + n ? ptrs[f] : ptrs[3];
+    ok = ok && encode_field_map<T>(h, &slot->maps.m[f], base, RS, ty + 2);
+  }
+  if (!ok) {
+    slot->ptrs.clear();
+    slot->stamp = 0;
+    return nullptr;
+  }
+  slot->ptrs = std::move(ptrs);
+  slot->ty = ty;
+  slot->stamp = ++h->map_clock;
+  return &slot->maps;
+}
+
 template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
 int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
                          const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(cudaFuncSetAttribute(tma_scalars<T, GW, ACC, SKEW, MOM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                          (int)pl.smem));
+  CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM>));
   dim3 grid(pl.tiles, pl.nchunks);
-  const int threads = (pl.ty * pl.zw * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
+  const int threads = (pl.ty * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
   CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
                 (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
@@ -401,27 +522,19 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
                     const void *const *q, void *const *sq, int nq, int ia, int ib,
                     cudaStream_t st, bool *done, const MomPtrs<T> *mo = nullptr) {
   *done = false;
-  constexpr int NK = VecOf<T>::NK;
   if (mo && nq > 10) return MONC_ADV_OK;
   for (int base = 0; base < nq; base += kMaxScalarsPerLaunch) {
     const int n = std::min(kMaxScalarsPerLaunch, nq - base);
-    const TmaScalarPlan pl = plan_tma_scalars<T>(h, ib - ia, n, mo != nullptr);
+    const TmaScalarPlan &pl = plan_tma_scalars<T>(h, ib - ia, n, mo != nullptr);
     if (!pl.ok) {
       if (base == 0) return MONC_ADV_OK;
       return fail(h, MONC_ADV_ECUDA, "scalars: TMA plan failed after a partial launch");
     }
-    const int RS = kRowBytes / (int)sizeof(T);
-    TensorMaps maps;
+    const TensorMaps *mp = field_maps<T>(h, u, v, w, q + base, n, pl.ty);
+    if (!mp) return fail(h, MONC_ADV_ECUDA, "scalars: cuTensorMapEncodeTiled failed");
+    const TensorMaps &maps = *mp;
     SqPtrs<T> outs;
-    bool ok = encode_field_map<T>(h, &maps.m[0], u, RS, pl.ty + 2) &&
-              encode_field_map<T>(h, &maps.m[1], v, RS, pl.ty + 2) &&
-              encode_field_map<T>(h, &maps.m[2], w, RS, pl.ty + 2);
-    for (int s = 0; s < kMaxScalarsPerLaunch; ++s) {
-      const int src = base + (s < n ? s : 0);
-      ok = ok && encode_field_map<T>(h, &maps.m[3 + s], q[src], RS, pl.ty + 2);
-      outs.sq[s] = (T *)sq[src];
-    }
-    if (!ok) return fail(h, MONC_ADV_ECUDA, "scalars: cuTensorMapEncodeTiled failed");
+    for (int s = 0; s < kMaxScalarsPerLaunch; ++s) outs.sq[s] = (T *)sq[base + (s < n ? s : 0)];
     p.xc = pl.xc;
     int rc = MONC_ADV_OK;
     switch (pl.gw) {
@@ -435,10 +548,9 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
     CU(cudaGetLastError());
     h->launches++;
     char b[200];
-    snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d zw=%d stages=%d xc=%d grid=%dx%d "
+    snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d stages=%d xc=%d grid=%dx%d "
              "threads=%d smem=%zu", mo ? "tma_fused(momentum+scalars)" : "tma_scalars", pl.gb, pl.gw, pl.ss,
-             pl.ty, pl.zw, pl.stages, pl.xc, pl.tiles, pl.nchunks,
-             (pl.ty * pl.zw * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
+             pl.ty, pl.stages, pl.xc, pl.tiles, pl.nchunks, (pl.ty * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
     h->plan_sca = b;
     if (mo) h->plan_mom.clear();
   }
@@ -565,9 +677,21 @@ int ensure_async_objects(monc_adv_t h, int nq) {
       // input planes beyond halo depth 1 are never copied: define them once
       CU(cudaMemset(h->d_in[n], 0, bytes));
     }
+    // the memsets run on the legacy default stream, which the internal (non-blocking)
+    // streams do not order against: finish them before any copy or kernel is queued
+    CU(cudaDeviceSynchronize());
     h->staged_nq = nq;
   }
   return MONC_ADV_OK;
+}
+
+// wait for whatever a failed enqueue left on the internal streams, so that the
+// caller's buffers are quiescent and the handle can be used again
+void drain_internal_streams(monc_adv_t h) {
+  if (h->s_in) cudaStreamSynchronize(h->s_in);
+  if (h->s_k) cudaStreamSynchronize(h->s_k);
+  if (h->s_out) cudaStreamSynchronize(h->s_out);
+  cudaGetLastError();
 }
 
 template <typename T>
@@ -612,6 +736,16 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
     const size_t off = (size_t)lo * plane_b, bytes = (size_t)(hi - lo) * plane_b;
     for (int n = 0; n < nf; ++n)
       CU(cudaMemcpyAsync((char *)h->d_in[n] + off, hin[n] + off, bytes, cudaMemcpyHostToDevice, sin));
+    if (h->accumulate) {
+      // accumulate: the caller's source terms of this slab go up too and the kernels add
+      // to them on the device, so what comes back is already combined
+      const int ia = h->h + h->chunk_a[c], ib = h->h + h->chunk_b[c];
+      const size_t ooff = ((size_t)ia * h->nyh + h->h) * h->nz * es;
+      const size_t width = (size_t)h->ny * h->nz * es;
+      for (int n = mom ? 0 : 3; n < nf; ++n)
+        CU(cudaMemcpy2DAsync((char *)h->d_out[n] + ooff, plane_b, hout[n] + ooff, plane_b, width,
+                             (size_t)(ib - ia), cudaMemcpyHostToDevice, sin));
+    }
     CU(cudaEventRecord(h->ev_h2d[c], sin));
     return MONC_ADV_OK;
   };
@@ -775,9 +909,8 @@ int monc_adv_momentum(monc_adv_t h, const void *u, const void *v, const void *w,
   const void *all[6] = {u, v, w, su, sv, sw};
   for (const void *p : all)
     if (!aligned16(p)) return fail(h, MONC_ADV_EINVAL, "momentum: pointers must be 16-byte aligned");
-  for (int a = 0; a < 3; ++a)
-    for (int b = 3; b < 6; ++b)
-      if (all[a] == all[b]) return fail(h, MONC_ADV_EINVAL, "momentum: inputs and outputs must not alias");
+  if (const char *why = find_alias({u, v, w}, {su, sv, sw}, h->elems * h->esize))
+    return fail(h, MONC_ADV_EINVAL, std::string("momentum: ") + why);
   h->wind[0] = u; h->wind[1] = v; h->wind[2] = w;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (h->dtype == MONC_ADV_F64)
@@ -795,15 +928,16 @@ int monc_adv_scalars(monc_adv_t h, const void *const *q, void *const *sq, int nq
   if (nq == 0) return MONC_ADV_OK;
   if (!q || !sq) return fail(h, MONC_ADV_EINVAL, "scalars: NULL pointer table");
   if (!h->wind[0]) return fail(h, MONC_ADV_ENOWIND, "scalars: no wind bound (call momentum or bind_wind first)");
+  std::vector<const void *> ins = {h->wind[0], h->wind[1], h->wind[2]}, outs;
   for (int n = 0; n < nq; ++n) {
     if (!q[n] || !sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: NULL field pointer");
     if (!aligned16(q[n]) || !aligned16(sq[n]))
       return fail(h, MONC_ADV_EINVAL, "scalars: pointers must be 16-byte aligned");
-    for (int m = 0; m < nq; ++m)
-      if (q[m] == sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: inputs and outputs must not alias");
-    for (int a = 0; a < 3; ++a)
-      if (h->wind[a] == sq[n]) return fail(h, MONC_ADV_EINVAL, "scalars: output aliases the wind");
+    ins.push_back(q[n]);
+    outs.push_back(sq[n]);
   }
+  if (const char *why = find_alias(ins, outs, h->elems * h->esize))
+    return fail(h, MONC_ADV_EINVAL, std::string("scalars: ") + why);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (h->dtype == MONC_ADV_F64)
     return launch_scalars<double>(h, (const double *)h->wind[0], (const double *)h->wind[1],
@@ -828,13 +962,10 @@ int monc_adv_tendencies(monc_adv_t h, const void *u, const void *v, const void *
   }
   for (const void *p : ins)
     if (!aligned16(p)) return fail(h, MONC_ADV_EINVAL, "tendencies: pointers must be 16-byte aligned");
-  for (size_t b = 0; b < outs.size(); ++b) {
-    if (!aligned16(outs[b])) return fail(h, MONC_ADV_EINVAL, "tendencies: pointers must be 16-byte aligned");
-    for (const void *a : ins)
-      if (a == outs[b]) return fail(h, MONC_ADV_EINVAL, "tendencies: inputs and outputs must not alias");
-    for (size_t c = 0; c < b; ++c)
-      if (outs[c] == outs[b]) return fail(h, MONC_ADV_EINVAL, "tendencies: outputs must be distinct");
-  }
+  for (const void *p : outs)
+    if (!aligned16(p)) return fail(h, MONC_ADV_EINVAL, "tendencies: pointers must be 16-byte aligned");
+  if (const char *why = find_alias(ins, outs, h->elems * h->esize))
+    return fail(h, MONC_ADV_EINVAL, std::string("tendencies: ") + why);
   h->wind[0] = u; h->wind[1] = v; h->wind[2] = w;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (h->dtype == MONC_ADV_F64)
@@ -864,12 +995,31 @@ int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void
   if (nq > 0 && (!hq || !hsq)) return fail(h, MONC_ADV_EINVAL, "step_async: NULL pointer table");
   for (int n = 0; n < nq; ++n)
     if (!hq[n] || !hsq[n]) return fail(h, MONC_ADV_EINVAL, "step_async: NULL field pointer");
+  std::vector<const void *> ins = {hu, hv, hw}, outs;
+  if (nout) outs = {hsu, hsv, hsw};
+  for (int n = 0; n < nq; ++n) { ins.push_back(hq[n]); outs.push_back(hsq[n]); }
+  const size_t bytes = h->elems * h->esize;
+  if (const char *why = find_alias(ins, outs, bytes))
+    return fail(h, MONC_ADV_EINVAL, std::string("step_async: ") + why);
+  for (const std::vector<const void *> *v : {&ins, &outs})
+    for (const void *p : *v)
+      if (!is_pinned_host(p, bytes))
+        return fail(h, MONC_ADV_EINVAL, "step_async: every host array must be page-locked (pinned) over its "
+                                        "whole length; pageable memory would make the copies synchronous");
   rc = ensure_async_objects(h, nq);
   if (rc) return rc;
   cudaStream_t user = (cudaStream_t)cuda_stream;
-  if (h->dtype == MONC_ADV_F64)
-    return step_async_impl<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
-  return step_async_impl<float>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
+  rc = h->dtype == MONC_ADV_F64 ? step_async_impl<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user)
+                                : step_async_impl<float>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
+  if (rc != MONC_ADV_OK) {
+    // part of the step may already be queued: let it finish (it touches only the caller's
+    // arrays of this call and the staging buffers), then report; the handle stays usable
+    const std::string msg = h->err;
+    drain_internal_streams(h);
+    h->in_flight = false;
+    h->err = msg;
+  }
+  return rc;
 }
 
 int monc_adv_step_inputs_consumed(monc_adv_t h) {
@@ -894,9 +1044,9 @@ int monc_adv_step_wait(monc_adv_t h) {
   if (rc) return rc;
   if (!h->in_flight) return MONC_ADV_OK;
   const int C = (int)h->chunk_a.size();
-  h->in_flight = false;
   CU(cudaEventSynchronize(h->ev_d2h[C - 1]));
   CU(cudaStreamSynchronize(h->s_in));
+  h->in_flight = false;  // only now: a failed wait leaves the step marked in flight
   float t = 0, ksum = 0;
   CU(cudaEventElapsedTime(&t, h->ev_in_begin, h->ev_h2d[C - 1]));
   h->times[0] = t;
@@ -981,6 +1131,8 @@ int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int w
   if (xchunk < 0 || group < 0 || group > 10 || prefetch < -1 || prefetch > 16 || warps < 0 ||
       warps > kWarpsPerBlock || stages < 0 || stages > 8 || tile_y < 0 || split < 0 || split > 4)
     return fail(h, MONC_ADV_EINVAL, "set_tuning: value out of range");
+  h->mom_plans.clear();
+  h->sca_plans.clear();
   h->split = split;
   h->stages = stages;
   h->tile_y = tile_y;

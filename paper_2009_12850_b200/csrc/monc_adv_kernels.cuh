@@ -20,7 +20,8 @@
 //              lines).  Every face flux is computed once per thread: the
 //              nine flux differences of the momentum equations need only six
 //              distinct products because the off-diagonal ones are shared
-//              (FxV == FyU, FxW == FzU, FyW == FzV).
+//              (FxV == FyU, FxW == FzU, FyW == FzV).  The arithmetic of one x
+//              step (momentum_faces) is shared with the TMA kernels.
 //
 // This header shares nothing with oracle/.
 #pragma once
@@ -143,58 +144,103 @@ __device__ __forceinline__ Vec<T> shift_down(const Vec<T> &f, int lane, T edge) 
   return r;
 }
 
-// ---------------------------------------------------------------------------
-// One x-step of the fused momentum update for one thread's NK levels.
-// Inputs: centre-plane values C/S/N, east-plane values E, the values one level
-// up (..u), the three fluxes below the thread's first level (b_*: from the
-// previous lane by shuffle, or `edge` values for lane 0) and the west-face
-// fluxes carried from the previous step.  Six distinct face fluxes per point:
-//   fxx (u_i+u_i+1)^2            fyy (v_j+v_j+1)^2           fzz (w_K+w_K+1)^2
-//   fxy (u_j+u_j+1)(v_i+v_i+1)   fxz (u_K+u_K+1)(w_i+w_i+1)  fyz (v_K+v_K+1)(w_j+w_j+1)
-// (FyU == FxV, FzU == FxW, FzV == FyW up to the constant).
-// On return fxx_w/fxy_w/fxz_w hold this step's EAST fluxes (next step's west).
-// ---------------------------------------------------------------------------
+// values of one x plane a thread carries to the next x step: u, v, w at its
+// column and v at the column to the south
 template <typename T>
-__device__ __forceinline__ void momentum_step(
-    const T cx, const T cy, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1,
-    const Vec<T> &d2, const Vec<T> &uC, const Vec<T> &vC, const Vec<T> &vS, const Vec<T> &wC,
+struct PlaneRegs {
+  Vec<T> u, v, vs, w;
+};
+// the three x-face fluxes carried to the next x step
+template <typename T>
+struct XFlux {
+  Vec<T> xx, xy, xz;
+};
+
+// ---------------------------------------------------------------------------
+// One x step of the fused momentum update for a thread's NK levels (SURVEY.md
+// 8(c).2 blocks su/sv/sw): centre plane RC, east plane RE, the centre plane's
+// south/north/upper neighbours, the west-face terms FW carried from the
+// previous step, and the three vertical fluxes b_* through the face below the
+// thread's first level that a shuffle cannot provide (lane 0; unused elsewhere).
+// Returns the tendencies of the centre plane and, in FE, the east-face terms
+// the next step needs as its west.
+// ---------------------------------------------------------------------------
+template <typename T, bool SKEW>
+__device__ __forceinline__ void momentum_faces(
+    const PlaneRegs<T> &RC, const PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE,
     const Vec<T> &uS, const Vec<T> &uN, const Vec<T> &vN, const Vec<T> &wS, const Vec<T> &wN,
-    const Vec<T> &uE, const Vec<T> &vE, const Vec<T> &vSE, const Vec<T> &wE, const Vec<T> &uCu,
-    const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const T b_xz, const T b_yz,
-    const T b_zz, const int lane, const int k0, const int nz, Vec<T> &fxx_w, Vec<T> &fxy_w,
-    Vec<T> &fxz_w, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
+    const Vec<T> &uCu, const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const T b_xz,
+    const T b_yz, const T b_zz, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1, const Vec<T> &d2,
+    const T cx, const T cy, const int lane, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
   constexpr int NK = VecOf<T>::NK;
-  Vec<T> fxx_e, fxy_e, fxz_e, fyz_n, fzz_t, ry, rv, rwy;
+  if (SKEW) {
+    // Piacsek-Williams skew form (R4): the advected parenthesis holds the
+    // neighbour's value only, so a face carries two products, A*phi_far for the
+    // point on this side and A*phi_near for the point across the face (handed on
+    // through FE in x, by shuffle in z), with the advecting sums A shared.
+    Vec<T> su_t, sv_t, sw_t, pu_t, pv_t, pw_t, ry, rv, rwy;
 #pragma unroll
-  for (int e = 0; e < NK; ++e) {
-    const T a = uC.v[e] + uE.v[e];
-    fxx_e.v[e] = a * a;                                              // centre i+1
-    fxy_e.v[e] = (uC.v[e] + uN.v[e]) * (vC.v[e] + vE.v[e]);          // corner (i+1/2, j+1/2)
-    const T fxy_se = (uS.v[e] + uC.v[e]) * (vS.v[e] + vSE.v[e]);     // corner (i+1/2, j-1/2)
-    fxz_e.v[e] = (uC.v[e] + uCu.v[e]) * (wC.v[e] + wE.v[e]);         // (i+1/2, z_K)
-    const T bn = vC.v[e] + vN.v[e], bs = vS.v[e] + vC.v[e];
-    fyz_n.v[e] = (vC.v[e] + vCu.v[e]) * (wC.v[e] + wN.v[e]);         // (j+1/2, z_K)
-    const T fyz_s = (vS.v[e] + vSu.v[e]) * (wS.v[e] + wC.v[e]);      // (j-1/2, z_K)
-    const T g = wC.v[e] + wCu.v[e];
-    fzz_t.v[e] = g * g;                                              // at zn_{K+1}
-    ry.v[e] = cy * (fxy_se - fxy_e.v[e]);                            // su: y
-    rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);                            // sw: y
-    rv.v[e] = cx * (fxy_w.v[e] - fxy_e.v[e]) + cy * (bs * bs - bn * bn);  // sv: x + y
-  }
-  const Vec<T> fxz_b = shift_down(fxz_e, lane, b_xz);
-  const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
-  const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
+    for (int e = 0; e < NK; ++e) {
+      const T axu = RC.u.v[e] + RE.u.v[e];     // advects u through the east face
+      const T axv = RC.u.v[e] + uN.v[e];       // advects v through the east face
+      const T axw = RC.u.v[e] + uCu.v[e];      // advects w through the east face
+      const T ayu_n = RC.v.v[e] + RE.v.v[e], ayu_s = RC.vs.v[e] + RE.vs.v[e];
+      const T ayv_n = RC.v.v[e] + vN.v[e], ayv_s = RC.vs.v[e] + RC.v.v[e];
+      const T ayw_n = RC.v.v[e] + vCu.v[e], ayw_s = RC.vs.v[e] + vSu.v[e];
+      const T azu = RC.w.v[e] + RE.w.v[e];     // advects u through the top face
+      const T azv = RC.w.v[e] + wN.v[e];
+      const T azw = RC.w.v[e] + wCu.v[e];
+      ry.v[e] = cx * (FW.xx.v[e] - axu * RE.u.v[e]) + cy * (ayu_s * uS.v[e] - ayu_n * uN.v[e]);
+      rv.v[e] = cx * (FW.xy.v[e] - axv * RE.v.v[e]) + cy * (ayv_s * RC.vs.v[e] - ayv_n * vN.v[e]);
+      rwy.v[e] = cx * (FW.xz.v[e] - axw * RE.w.v[e]) + cy * (ayw_s * wS.v[e] - ayw_n * wN.v[e]);
+      FE.xx.v[e] = axu * RC.u.v[e];
+      FE.xy.v[e] = axv * RC.v.v[e];
+      FE.xz.v[e] = axw * RC.w.v[e];
+      su_t.v[e] = azu * uCu.v[e]; pu_t.v[e] = azu * RC.u.v[e];
+      sv_t.v[e] = azv * vCu.v[e]; pv_t.v[e] = azv * RC.v.v[e];
+      sw_t.v[e] = azw * wCu.v[e]; pw_t.v[e] = azw * RC.w.v[e];
+    }
+    const Vec<T> fu_b = shift_down(pu_t, lane, b_xz);
+    const Vec<T> fv_b = shift_down(pv_t, lane, b_yz);
+    const Vec<T> fw_b = shift_down(pw_t, lane, b_zz);
 #pragma unroll
-  for (int e = 0; e < NK; ++e) {
-    const int k = k0 + e;
-    T xu = cx * (fxx_w.v[e] - fxx_e.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * fxz_e.v[e]);
-    T xv = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
-    T xw = cx * (fxz_w.v[e] - fxz_e.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
-    if (k == 0) { xu = T(0); xv = T(0); xw = T(0); }
-    if (k == nz - 1) xw = T(0);
-    ou.v[e] = xu; ov.v[e] = xv; ow.v[e] = xw;
+    for (int e = 0; e < NK; ++e) {
+      ou.v[e] = ry.v[e] + (c1.v[e] * fu_b.v[e] - c2.v[e] * su_t.v[e]);
+      ov.v[e] = rv.v[e] + (c1.v[e] * fv_b.v[e] - c2.v[e] * sv_t.v[e]);
+      ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
+    }
+  } else {
+    // six distinct face fluxes:
+    //   fxx (u_i+u_i+1)^2            fyy (v_j+v_j+1)^2           fzz (w_K+w_K+1)^2
+    //   fxy (u_j+u_j+1)(v_i+v_i+1)   fxz (u_K+u_K+1)(w_i+w_i+1)  fyz (v_K+v_K+1)(w_j+w_j+1)
+    // (FyU == FxV, FzU == FxW, FzV == FyW up to the constant)
+    Vec<T> fyz_n, fzz_t, ry, rv, rwy;
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      const T a = RC.u.v[e] + RE.u.v[e];
+      FE.xx.v[e] = a * a;
+      FE.xy.v[e] = (RC.u.v[e] + uN.v[e]) * (RC.v.v[e] + RE.v.v[e]);
+      const T fxy_se = (uS.v[e] + RC.u.v[e]) * (RC.vs.v[e] + RE.vs.v[e]);
+      FE.xz.v[e] = (RC.u.v[e] + uCu.v[e]) * (RC.w.v[e] + RE.w.v[e]);
+      const T bn = RC.v.v[e] + vN.v[e], bs = RC.vs.v[e] + RC.v.v[e];
+      fyz_n.v[e] = (RC.v.v[e] + vCu.v[e]) * (RC.w.v[e] + wN.v[e]);
+      const T fyz_s = (RC.vs.v[e] + vSu.v[e]) * (wS.v[e] + RC.w.v[e]);
+      const T g = RC.w.v[e] + wCu.v[e];
+      fzz_t.v[e] = g * g;
+      ry.v[e] = cy * (fxy_se - FE.xy.v[e]);
+      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);
+      rv.v[e] = cx * (FW.xy.v[e] - FE.xy.v[e]) + cy * (bs * bs - bn * bn);
+    }
+    const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
+    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
+    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
+#pragma unroll
+    for (int e = 0; e < NK; ++e) {
+      ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
+      ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
+      ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
+    }
   }
-  fxx_w = fxx_e; fxy_w = fxy_e; fxz_w = fxz_e;
 }
 
 // ---------------------------------------------------------------------------
@@ -235,11 +281,12 @@ march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict_
   const T *pu = u + c0, *pv = v + c0, *pw = w + c0;
   T *qu = su + c0, *qv = sv + c0, *qw = sw + c0;
   // values of the centre plane that the previous step already loaded
-  Vec<T> uC = ld_vec(pu), vC = ld_vec(pv), vS = ld_vec(pv - nz), wC = ld_vec(pw);
+  PlaneRegs<T> RC, RE;
+  RC.u = ld_vec(pu); RC.v = ld_vec(pv); RC.vs = ld_vec(pv - nz); RC.w = ld_vec(pw);
   // x-face fluxes on the west side, carried from the previous step
-  Vec<T> fxx_w, fxy_w, fxz_w;
+  XFlux<T> FW, FE;
 #pragma unroll
-  for (int e = 0; e < NK; ++e) fxx_w.v[e] = fxy_w.v[e] = fxz_w.v[e] = T(0);
+  for (int e = 0; e < NK; ++e) FW.xx.v[e] = FW.xy.v[e] = FW.xz.v[e] = T(0);
   const int pf = p.prefetch;
   // one lane per warp asks the TMA unit to pull this warp's 32 vectors of
   // plane i+pf into L2 (DRAM latency then overlaps the steps in between)
@@ -251,8 +298,8 @@ march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict_
     const Vec<T> uS = ld_vec(pu - nz), uN = ld_vec(pu + nz);
     const Vec<T> vN = ld_vec(pv + nz);
     const Vec<T> wS = ld_vec(pw - nz), wN = ld_vec(pw + nz);
-    const Vec<T> uE = ld_vec(pu + plane), vE = ld_vec(pv + plane);
-    const Vec<T> vSE = ld_vec(pv + plane - nz), wE = ld_vec(pw + plane);
+    RE.u = ld_vec(pu + plane); RE.v = ld_vec(pv + plane);
+    RE.vs = ld_vec(pv + plane - nz); RE.w = ld_vec(pw + plane);
     if (pf_lane && i + pf <= i1) {  // pull plane i+pf of this column towards L2
       prefetch_l2_bulk(pu + pf * plane, pf_bytes); prefetch_l2_bulk(pv + pf * plane, pf_bytes);
       prefetch_l2_bulk(pw + pf * plane, pf_bytes);
@@ -268,18 +315,19 @@ march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict_
       if (bot_edge) {
         const T ub = __ldg(pu - 1), vb = __ldg(pv - 1), wb = __ldg(pw - 1);
         const T web = __ldg(pw + plane - 1), wnb = __ldg(pw + nz - 1);
-        b_xz = (ub + uC.v[0]) * (wb + web);
-        b_yz = (vb + vC.v[0]) * (wb + wnb);
-        b_zz = (wb + wC.v[0]) * (wb + wC.v[0]);
+        b_xz = (ub + RC.u.v[0]) * (wb + web);
+        b_yz = (vb + RC.v.v[0]) * (wb + wnb);
+        b_zz = (wb + RC.w.v[0]) * (wb + RC.w.v[0]);
       }
     }
-    const Vec<T> uCu = shift_up(uC, lane, e_u), vCu = shift_up(vC, lane, e_v);
-    const Vec<T> wCu = shift_up(wC, lane, e_w), vSu = shift_up(vS, lane, e_vs);
+    const Vec<T> uCu = shift_up(RC.u, lane, e_u), vCu = shift_up(RC.v, lane, e_v);
+    const Vec<T> wCu = shift_up(RC.w, lane, e_w), vSu = shift_up(RC.vs, lane, e_vs);
 
     Vec<T> ou, ov, ow;
-    momentum_step<T>(cx, cy, c1, c2, d1, d2, uC, vC, vS, wC, uS, uN, vN, wS, wN, uE, vE, vSE, wE,
-                     uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, lane, k0, nz, fxx_w, fxy_w, fxz_w, ou,
-                     ov, ow);
+    momentum_faces<T, false>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz,
+                             c1, c2, d1, d2, cx, cy, lane, ou, ov, ow);
+    if (k0 == 0) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }  // level K = 1: no tendency
+    if (k0 + NK == nz) ow.v[NK - 1] = T(0);                            // level K = nz: sw = 0
     if (i >= i0 && act) {
       if (p.accumulate) {
         const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
@@ -288,8 +336,9 @@ march_momentum(const KParams<T> p, const T *__restrict__ u, const T *__restrict_
       }
       st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
     }
-    // rotate: east becomes centre
-    uC = uE; vC = vE; vS = vSE; wC = wE;
+    // rotate: east becomes centre, its x-face terms the next step's west
+    RC = RE;
+    FW = FE;
     pu += plane; pv += plane; pw += plane;
     qu += plane; qv += plane; qw += plane;
   }

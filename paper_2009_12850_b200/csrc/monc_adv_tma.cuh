@@ -130,105 +130,6 @@ __device__ __forceinline__ float keep_if(float x, int m) {
   return __int_as_float(__float_as_int(x) & m);
 }
 
-// values of one x plane a thread carries to the next x step: u, v, w at its
-// column and v at the column to the south
-template <typename T>
-struct PlaneRegs {
-  Vec<T> u, v, vs, w;
-};
-// the three x-face fluxes carried to the next x step
-template <typename T>
-struct XFlux {
-  Vec<T> xx, xy, xz;
-};
-
-// ---------------------------------------------------------------------------
-// One x step of the fused momentum update for a thread's NK levels (SURVEY.md
-// 8(c).2 blocks su/sv/sw): centre plane RC, east plane RE, the centre plane's
-// south/north/upper neighbours, the west-face terms FW carried from the
-// previous step, and the three vertical fluxes b_* through the face below the
-// thread's first level that a shuffle cannot provide (lane 0; unused elsewhere).
-// Returns the tendencies of the centre plane and, in FE, the east-face terms
-// the next step needs as its west.
-// ---------------------------------------------------------------------------
-template <typename T, bool SKEW>
-__device__ __forceinline__ void momentum_faces(
-    const PlaneRegs<T> &RC, const PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE,
-    const Vec<T> &uS, const Vec<T> &uN, const Vec<T> &vN, const Vec<T> &wS, const Vec<T> &wN,
-    const Vec<T> &uCu, const Vec<T> &vCu, const Vec<T> &wCu, const Vec<T> &vSu, const T b_xz,
-    const T b_yz, const T b_zz, const Vec<T> &c1, const Vec<T> &c2, const Vec<T> &d1, const Vec<T> &d2,
-    const T cx, const T cy, const int lane, Vec<T> &ou, Vec<T> &ov, Vec<T> &ow) {
-  constexpr int NK = VecOf<T>::NK;
-  if (SKEW) {
-    // Piacsek-Williams skew form (R4): the advected parenthesis holds the
-    // neighbour's value only, so a face carries two products, A*phi_far for the
-    // point on this side and A*phi_near for the point across the face (handed on
-    // through FE in x, by shuffle in z), with the advecting sums A shared.
-    Vec<T> su_t, sv_t, sw_t, pu_t, pv_t, pw_t, ry, rv, rwy;
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      const T axu = RC.u.v[e] + RE.u.v[e];     // advects u through the east face
-      const T axv = RC.u.v[e] + uN.v[e];       // advects v through the east face
-      const T axw = RC.u.v[e] + uCu.v[e];      // advects w through the east face
-      const T ayu_n = RC.v.v[e] + RE.v.v[e], ayu_s = RC.vs.v[e] + RE.vs.v[e];
-      const T ayv_n = RC.v.v[e] + vN.v[e], ayv_s = RC.vs.v[e] + RC.v.v[e];
-      const T ayw_n = RC.v.v[e] + vCu.v[e], ayw_s = RC.vs.v[e] + vSu.v[e];
-      const T azu = RC.w.v[e] + RE.w.v[e];     // advects u through the top face
-      const T azv = RC.w.v[e] + wN.v[e];
-      const T azw = RC.w.v[e] + wCu.v[e];
-      ry.v[e] = cx * (FW.xx.v[e] - axu * RE.u.v[e]) + cy * (ayu_s * uS.v[e] - ayu_n * uN.v[e]);
-      rv.v[e] = cx * (FW.xy.v[e] - axv * RE.v.v[e]) + cy * (ayv_s * RC.vs.v[e] - ayv_n * vN.v[e]);
-      rwy.v[e] = cx * (FW.xz.v[e] - axw * RE.w.v[e]) + cy * (ayw_s * wS.v[e] - ayw_n * wN.v[e]);
-      FE.xx.v[e] = axu * RC.u.v[e];
-      FE.xy.v[e] = axv * RC.v.v[e];
-      FE.xz.v[e] = axw * RC.w.v[e];
-      su_t.v[e] = azu * uCu.v[e]; pu_t.v[e] = azu * RC.u.v[e];
-      sv_t.v[e] = azv * vCu.v[e]; pv_t.v[e] = azv * RC.v.v[e];
-      sw_t.v[e] = azw * wCu.v[e]; pw_t.v[e] = azw * RC.w.v[e];
-    }
-    const Vec<T> fu_b = shift_down(pu_t, lane, b_xz);
-    const Vec<T> fv_b = shift_down(pv_t, lane, b_yz);
-    const Vec<T> fw_b = shift_down(pw_t, lane, b_zz);
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      ou.v[e] = ry.v[e] + (c1.v[e] * fu_b.v[e] - c2.v[e] * su_t.v[e]);
-      ov.v[e] = rv.v[e] + (c1.v[e] * fv_b.v[e] - c2.v[e] * sv_t.v[e]);
-      ow.v[e] = rwy.v[e] + (d1.v[e] * fw_b.v[e] - d2.v[e] * sw_t.v[e]);
-    }
-  } else {
-    // six distinct face fluxes:
-    //   fxx (u_i+u_i+1)^2            fyy (v_j+v_j+1)^2           fzz (w_K+w_K+1)^2
-    //   fxy (u_j+u_j+1)(v_i+v_i+1)   fxz (u_K+u_K+1)(w_i+w_i+1)  fyz (v_K+v_K+1)(w_j+w_j+1)
-    // (FyU == FxV, FzU == FxW, FzV == FyW up to the constant)
-    Vec<T> fyz_n, fzz_t, ry, rv, rwy;
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      const T a = RC.u.v[e] + RE.u.v[e];
-      FE.xx.v[e] = a * a;
-      FE.xy.v[e] = (RC.u.v[e] + uN.v[e]) * (RC.v.v[e] + RE.v.v[e]);
-      const T fxy_se = (uS.v[e] + RC.u.v[e]) * (RC.vs.v[e] + RE.vs.v[e]);
-      FE.xz.v[e] = (RC.u.v[e] + uCu.v[e]) * (RC.w.v[e] + RE.w.v[e]);
-      const T bn = RC.v.v[e] + vN.v[e], bs = RC.vs.v[e] + RC.v.v[e];
-      fyz_n.v[e] = (RC.v.v[e] + vCu.v[e]) * (RC.w.v[e] + wN.v[e]);
-      const T fyz_s = (RC.vs.v[e] + vSu.v[e]) * (wS.v[e] + RC.w.v[e]);
-      const T g = RC.w.v[e] + wCu.v[e];
-      fzz_t.v[e] = g * g;
-      ry.v[e] = cy * (fxy_se - FE.xy.v[e]);
-      rwy.v[e] = cy * (fyz_s - fyz_n.v[e]);
-      rv.v[e] = cx * (FW.xy.v[e] - FE.xy.v[e]) + cy * (bs * bs - bn * bn);
-    }
-    const Vec<T> fxz_b = shift_down(FE.xz, lane, b_xz);
-    const Vec<T> fyz_b = shift_down(fyz_n, lane, b_yz);
-    const Vec<T> fzz_b = shift_down(fzz_t, lane, b_zz);
-#pragma unroll
-    for (int e = 0; e < NK; ++e) {
-      ou.v[e] = cx * (FW.xx.v[e] - FE.xx.v[e]) + ry.v[e] + (c1.v[e] * fxz_b.v[e] - c2.v[e] * FE.xz.v[e]);
-      ov.v[e] = rv.v[e] + (c1.v[e] * fyz_b.v[e] - c2.v[e] * fyz_n.v[e]);
-      ow.v[e] = cx * (FW.xz.v[e] - FE.xz.v[e]) + rwy.v[e] + (d1.v[e] * fzz_b.v[e] - d2.v[e] * fzz_t.v[e]);
-    }
-  }
-}
-
 // ---------------------------------------------------------------------------
 // momentum_march: the x march of one warp over its column chunk, fed by a ring
 // of staged planes.  Used by tma_momentum (every consumer warp) and by the

@@ -102,6 +102,31 @@ def exchange_halo_x(fields, halo: int, depth: int | None = None, group=None):
     return None
 
 
+def exchange_halo_x_same_device(slabs, halo: int, depth: int | None = None):
+    """The same periodic swap for several sub-domains that live in ONE process on ONE
+    device (the paper runs 8 ranks per GPU; with a single GPU it
+    is also how the decomposed path is exercised on hardware): `slabs[r]` is the
+    list of field tensors of sub-domain r, ring order.  Planes move by
+    device-to-device copies on the current stream, straight from the neighbour's
+    edge planes into the rim: the data motion `exchange_halo_x` performs with
+    isend/irecv, minus the wire."""
+    depth = halo if depth is None else depth
+    if not 1 <= depth <= halo:
+        raise ValueError("need 1 <= depth <= halo")
+    world = len(slabs)
+    for r in range(world):
+        east = slabs[(r + 1) % world]
+        for f, fe in zip(slabs[r], east):
+            if not (f.is_contiguous() and fe.is_contiguous()):
+                raise ValueError("exchange_halo_x_same_device needs contiguous fields")
+            nxl, nxe = f.shape[0] - 2 * halo, fe.shape[0] - 2 * halo
+            if min(nxl, nxe) < depth:
+                raise ValueError("slab thinner than the halo depth")
+            fe[halo - depth:halo].copy_(f[nxl + halo - depth:nxl + halo], non_blocking=True)  # my last planes -> east's west rim
+            f[nxl + halo:nxl + halo + depth].copy_(fe[halo:halo + depth], non_blocking=True)   # east's first planes -> my east rim
+    return None
+
+
 def max_over_ranks(value: float, device="cpu", group=None) -> float:
     """Timing rule: a multi-rank number is the MAX over ranks."""
     if not dist.is_initialized() or dist.get_world_size(group) == 1:

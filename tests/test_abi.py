@@ -12,6 +12,7 @@ from paper_2009_12850_b200 import build as libbuild
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "monc_adv.h")
+TUNING_HEADER = os.path.join(ROOT, "include", "monc_adv_tuning.h")  # internal knobs, same library
 
 
 @pytest.fixture(scope="module")
@@ -20,18 +21,24 @@ def lib():
     return binding.load()
 
 
-def declared_functions():
-    src = open(HEADER).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(monc_adv_[a-z_0-9]+)\s*\(", src)))
+def declared_functions(headers=(HEADER, TUNING_HEADER)):
+    names = set()
+    for path in headers:
+        src = re.sub(r"/\*.*?\*/", "", open(path).read(), flags=re.S)
+        names |= set(re.findall(r"\b(monc_adv_[a-z_0-9]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_header_symbols_all_exported(lib):
     names = declared_functions()
     assert len(names) >= 20
     for n in names:
-        assert hasattr(lib, n), f"{n} declared in monc_adv.h but not exported"
-    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of sync with the header"
+        assert hasattr(lib, n), f"{n} declared in include/ but not exported"
+    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of sync with the headers"
+    # the kernel-geometry knobs live in the internal header only
+    public = declared_functions((HEADER,))
+    for n in ("monc_adv_set_tuning", "monc_adv_set_variant", "monc_adv_set_pdl"):
+        assert n not in public and n in names
 
 
 def test_version_string(lib):

@@ -92,3 +92,27 @@ def test_single_rank_wrap_and_ranges():
         pd.slab_range(2, 3, 0)
     with pytest.raises(ValueError):
         pd.exchange_halo_x([f], 2, depth=3)
+
+
+@pytest.mark.parametrize("world,nx,depth", [(2, 9, 2), (3, 11, 1), (4, 8, 2)])
+def test_same_device_slab_swap_matches_single_domain(world, nx, depth):
+    """Several sub-domains in one process (8 ranks share a GPU): the rims
+    filled by exchange_halo_x_same_device equal the single-domain periodic halos."""
+    sys.path.insert(0, ROOT)
+    from paper_2009_12850_b200 import dist as pd, synth
+    cfg = synth.Config(79, nx, 5, 6, halo=2, nq=1)
+    h = cfg.halo
+    names = ["u", "theta"]
+    G = {n: synth.interior_field(cfg, n) for n in names}
+    slabs = []
+    for r in range(world):
+        fs = [pd.local_from_global(G[n], h, world, r) for n in names]
+        for f in fs:
+            pd.fill_halo_y_periodic(f, h)
+        slabs.append(fs)
+    pd.exchange_halo_x_same_device(slabs, h, depth=depth)
+    for r in range(world):
+        x0, x1 = pd.slab_range(nx, world, r)
+        for n, f in zip(names, slabs[r]):
+            want = synth.embed(G[n], h)[x0 + h - depth:x1 + h + depth]
+            assert np.array_equal(f.numpy()[h - depth:h + (x1 - x0) + depth], want)

@@ -122,116 +122,166 @@ def test_step_async_after_user_stream_work():
 
 # ---------------------------------------------------------------------------
 # BASELINE.json configs 2, 3 (512x512x256, 3 momentum + 10 scalars) at full
-# size: every output field checked on sampled points the oracle computes one
-# by one, plus one x-slab compared element by element.
+# size, in the launch configuration bench.py times: EVERY interior element of
+# all 13 outputs, of the two north_star calls and of the fused launch, against
+# the oracle (threaded over the host cores: a full pass costs seconds).
 # ---------------------------------------------------------------------------
-def _big_fields(cfg):
-    U, V, W = [synth.field(cfg, n) for n in "uvw"]
-    names = synth.field_names(cfg)
-    return U, V, W, names
-
-
 @pytest.mark.parametrize("cid", [2, 3])
-def test_config2_and_3_full_size_sampled(cid):
+def test_config2_and_3_full_size_every_element(cid):
     cfg = synth.CONFIGS[cid]
     P, L = gc.make_pair(cfg)
-    U, V, W, names = _big_fields(cfg)
+    nthr = oracle.max_threads()
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    names = synth.field_names(cfg)
     d = [gc.to_dev(a, L) for a in (U, V, W)]
-    outs = gc.fresh_out(L, 3)
-    L.momentum(*d, *outs)
-    torch.cuda.synchronize()
-    rng = np.random.default_rng(cid)
-    ii, jj, kk = gc.sample_points(cfg, 40000, rng)
-    # scale: max |tendency| of the field, from the oracle on one x-slab (>= 8 planes)
-    slab = dataclasses.replace(cfg, nx=8)
-    Ps = oracle.Problem(slab.nx, slab.ny, slab.nz, slab.halo, synth.DX, synth.DY,
-                        *[synth.grid(cfg.nz)[k] for k in ("dz", "dzn", "rho", "rhon")])
-    sl = slice(100, 100 + 8 + 2 * cfg.halo)
-    Us, Vs, Ws = (np.ascontiguousarray(a[sl]) for a in (U, V, W))
-    want_slab = Ps.momentum(Us, Vs, Ws, nthreads=oracle.max_threads())
-    for o, w_, n in zip(outs, want_slab, ("su", "sv", "sw")):
-        scale = np.abs(gc.interior(slab, w_)).max()
-        gc.check_sampled(cfg, P, n, o, U, V, W, None, ii, jj, kk, scale)
-        # the slab, element by element (columns are independent: PAPER.md:73)
-        got = o[sl].cpu().numpy()
-        gc.check(slab, got, w_, n + "[slab]")
-    outs_m, scales = outs, [np.abs(gc.interior(slab, w_)).max() for w_ in want_slab]
-    # scalars, all nq in one batched call
-    outs = gc.fresh_out(L, cfg.nq)
-    dq = []
-    for n in names:
-        dq.append(gc.to_dev(synth.field(cfg, n), L))
-    L.scalars(dq, outs)
-    torch.cuda.synchronize()
-    for n, o, q in zip(names, outs, dq):
-        Q = synth.field(cfg, n)
-        qs = np.ascontiguousarray(Q[sl])
-        w_ = Ps.scalar(Us, Vs, Ws, qs, nthreads=oracle.max_threads())
-        scale = np.abs(gc.interior(slab, w_)).max()
-        gc.check_sampled(cfg, P, n, o, U, V, W, Q, ii, jj, kk, scale)
-        gc.check(slab, o[sl].cpu().numpy(), w_, n + "[slab]")
-        scales.append(scale)
-    # the whole step through monc_adv_tendencies (the launch bench.py times as the
-    # headline of this config): ONE fused launch, every element within tolerance of the
-    # two-call results just checked against the oracle
+    dq = [gc.to_dev(synth.field(cfg, n), L) for n in names]
+    two = gc.fresh_out(L, 3 + cfg.nq)
+    L.momentum(*d, *two[:3])
+    L.scalars(dq, two[3:])
+    assert "tma_momentum" in L.describe_plan() and "tma_scalars" in L.describe_plan(), L.describe_plan()
+    # the whole step through monc_adv_tendencies (bench.py's headline): ONE fused launch
     fo = gc.fresh_out(L, 3 + cfg.nq)
     L.tendencies(*d, fo[0], fo[1], fo[2], dq, fo[3:])
     torch.cuda.synchronize()
     assert "tma_fused" in L.describe_plan(), L.describe_plan()
-    h = cfg.halo
-    for a, b, sc, n in zip(fo, list(outs_m) + list(outs), scales, ["su", "sv", "sw"] + list(names)):
-        ai, bi = (t[h:h + cfg.nx, h:h + cfg.ny] for t in (a, b))
-        err = float((ai - bi).abs().max()) / sc
-        assert err <= gc.TOL[cfg.dtype], f"{n}: fused vs two calls {err:.3e}"
-        gc.check_sampled(cfg, P, n if n in ("su", "sv", "sw") else n, a, U, V, W,
-                         None if n in ("su", "sv", "sw") else synth.field(cfg, n), ii, jj, kk, sc)
+    errs = {}
+    want = P.momentum(U, V, W, nthreads=nthr)
+    for idx, nm in enumerate(("su", "sv", "sw")):
+        errs[nm] = (gc.check(cfg, two[idx], want[idx], nm + "[two calls]"),
+                    gc.check(cfg, fo[idx], want[idx], nm + "[fused]"))
+        gc.check_halo_untouched(cfg, two[idx], nm)
+        gc.check_halo_untouched(cfg, fo[idx], nm)
+    del want
+    sq = np.zeros(P.shape)
+    for idx, nm in enumerate(names):
+        P.scalar(U, V, W, synth.field(cfg, nm), nthreads=nthr, out=sq)
+        errs[nm] = (gc.check(cfg, two[3 + idx], sq, nm + "[two calls]"),
+                    gc.check(cfg, fo[3 + idx], sq, nm + "[fused]"))
+        gc.check_halo_untouched(cfg, fo[3 + idx], nm)
+    print(f"config{cid} full-array max rel errs (two calls, fused):",
+          {k: (f"{a:.1e}", f"{b:.1e}") for k, (a, b) in errs.items()})
     L.close()
 
 
 def test_config4_hybrid_async_full_size():
-    """1024x1024x160, 3 momentum + 4 scalars in pinned host memory, 8 chunks.
-    The seeded fields are perturbed every step; steps checked
-    against the oracle on sampled points and one x-slab."""
+    """1024x1024x160, 3 momentum + 4 scalars in pinned host memory, 8 chunks, the
+    20-step loop of BASELINE.json configs[4]: the seeded fields are perturbed every
+    step; steps 1, 10 and 20 are compared with the oracle on EVERY
+    interior element of all 7 outputs (chunk seams included)."""
     cfg = synth.CONFIGS[4]
-    steps_checked = (1, 2, 3)
+    steps_checked = (1, 10, 20)
     P, L = gc.make_pair(cfg)
     L.set_chunks(8)
+    nthr = oracle.max_threads()
     names = ["u", "v", "w"] + synth.field_names(cfg)
-    H = [synth.field(cfg, n) for n in names]
-    hin = [pinned(a, L) for a in H]
+    hin = [pinned(synth.field(cfg, n), L) for n in names]
     hout = pinned_out(L, len(names))
-    rng = np.random.default_rng(4)
-    slab = dataclasses.replace(cfg, nx=4)
-    g = synth.grid(cfg.nz)
-    Ps = oracle.Problem(slab.nx, slab.ny, slab.nz, slab.halo, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"])
-    for step in range(1, max(steps_checked) + 1):
+    sq = np.zeros(P.shape)
+    for step in range(1, cfg.steps + 1):
+        if step > 1:
+            L.step_inputs_consumed()   # the host may overwrite its fields once the H2D copies are done
+            L.step_wait()
         for n, t in zip(names, hin):
             synth.perturb(cfg, n, t.numpy(), step)   # in place on the pinned inputs
         L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
-        L.step_inputs_consumed()
-        L.step_wait()
         if step not in steps_checked:
             continue
+        L.step_wait()
+        assert "tma_fused" in L.describe_plan(), L.describe_plan()
         U, V, W = (t.numpy() for t in hin[:3])
-        ii, jj, kk = gc.sample_points(cfg, 20000, rng)
-        # chunk seams along x: sample planes next to every chunk boundary
-        seams = [L.step_chunk_range(c)[0] + cfg.halo for c in range(1, 8)]
-        ii[:2000] = np.array(seams + [s - 1 for s in seams])[rng.integers(0, 14, 2000)]
-        sl = slice(381, 381 + 4 + 2 * cfg.halo)   # straddles the chunk seam at x = 384
-        Us, Vs, Ws = (np.ascontiguousarray(a[sl]) for a in (U, V, W))
-        wm = Ps.momentum(Us, Vs, Ws, nthreads=oracle.max_threads())
-        for idx, n in enumerate(names):
-            if idx < 3:
-                w_ = wm[idx]
-                q = None
-                nm = ("su", "sv", "sw")[idx]
-            else:
-                q = hin[idx].numpy()
-                w_ = Ps.scalar(Us, Vs, Ws, np.ascontiguousarray(q[sl]), nthreads=oracle.max_threads())
-                nm = n
-            scale = np.abs(gc.interior(slab, w_)).max()
-            gc.check_sampled(cfg, P, nm, hout[idx].numpy(), U, V, W, q, ii, jj, kk, scale)
-            gc.check(slab, hout[idx].numpy()[sl], w_, nm + "[slab]")
-    t = L.step_times_ms()
-    print("config4 step times (ms):", t)
+        errs = {}
+        wm = P.momentum(U, V, W, nthreads=nthr)
+        for idx, nm in enumerate(("su", "sv", "sw")):
+            errs[nm] = gc.check(cfg, hout[idx].numpy(), wm[idx], f"{nm}[step {step}]")
+        del wm
+        for idx in range(3, len(names)):
+            P.scalar(U, V, W, hin[idx].numpy(), nthreads=nthr, out=sq)
+            errs[names[idx]] = gc.check(cfg, hout[idx].numpy(), sq, f"{names[idx]}[step {step}]")
+        print(f"config4 step {step} full-array max rel errs:", {k: f"{v:.1e}" for k, v in errs.items()})
+    for o, n in zip(hout, names):
+        gc.check_halo_untouched(cfg, o, n)
+    print("config4 step times (ms):", L.step_times_ms())
+    L.close()
+
+
+# ---------------------------------------------------------------------------
+# accumulate inside the hybrid step (SURVEY.md 8(f) NEXT-2; PAPER.md:99-101, 151):
+# the host's own source terms go up with the fields, the advection tendencies are
+# added on the device, the combined terms come back into the same arrays
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_step_async_accumulate_is_bitwise_wait_then_add(dtype):
+    cfg = gc.custom_cfg(22, 13, 96, nq=3, dtype=dtype, cid=404)
+    P, L = gc.make_pair(cfg)
+    L.set_chunks(4)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    hin = [pinned(synth.field(cfg, n), L) for n in names]
+    # wait-all-then-add: the plain step into a separate result buffer, host adds
+    plain = pinned_out(L, len(names))
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], plain[0], plain[1], plain[2], plain[3:])
+    L.step_wait()
+    rng = np.random.default_rng(5)
+    host_terms = [torch.from_numpy(rng.standard_normal(L.shape)).to(L.torch_dtype) for _ in names]
+    acc = [pinned(t.numpy(), L) for t in host_terms]
+    L.set_accumulate(True)
+    h = cfg.halo
+    sl = (slice(h, h + cfg.nx), slice(h, h + cfg.ny))
+    for rep in (1, 2):   # twice: the staging buffers must not carry step 1 into step 2
+        base = [a_.clone() for a_ in acc]
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], acc[0], acc[1], acc[2], acc[3:])
+        for c in range(4):   # streaming combine: a chunk's slab is final when its event fires
+            L.step_wait_chunk(c)
+            a, b = L.step_chunk_range(c)
+            xs = slice(h + a, h + b)
+            assert torch.equal(acc[0][xs, sl[1]], base[0][xs, sl[1]] + plain[0][xs, sl[1]])
+        L.step_wait()
+        for b_, a_, p_ in zip(base, acc, plain):
+            assert torch.equal(a_[sl], b_[sl] + p_[sl])   # bitwise: the same add, done on the device
+            m = torch.ones(L.shape, dtype=torch.bool)
+            m[sl] = False
+            assert torch.equal(a_[m], b_[m])              # halos untouched
+    # scalars only, accumulate still on
+    acc2 = [pinned(t.numpy(), L) for t in host_terms[3:]]
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], None, None, None, acc2)
+    L.step_wait()
+    for t0, a_, p_ in zip(host_terms[3:], acc2, plain[3:]):
+        assert torch.equal(a_[sl], t0[sl] + p_[sl])
+    L.close()
+
+
+# ---------------------------------------------------------------------------
+# the boundary refuses what would silently change the behaviour (C ABI called
+# directly, without the binding's own checks)
+# ---------------------------------------------------------------------------
+def test_step_async_refuses_pageable_and_overlapping_arrays():
+    import ctypes as C
+    cfg = gc.custom_cfg(8, 6, 32, nq=1, cid=405)
+    P, L = gc.make_pair(cfg)
+    lib, hd = L._lib, L._h
+    vp = C.c_void_p
+    pin = [torch.zeros(L.shape, dtype=L.torch_dtype).pin_memory() for _ in range(8)]
+    pageable = torch.zeros(L.shape, dtype=L.torch_dtype)
+
+    def call(hu, hv, hw, hq, hsu, hsv, hsw, hsq):
+        qt = (vp * 1)(hq.data_ptr())
+        st = (vp * 1)(hsq.data_ptr())
+        return lib.monc_adv_step_async(hd, vp(hu.data_ptr()), vp(hv.data_ptr()), vp(hw.data_ptr()), qt, 1,
+                                       vp(hsu.data_ptr()), vp(hsv.data_ptr()), vp(hsw.data_ptr()), st, None)
+
+    # PAPER.md:95: "silently reverting from an asynchronous to a synchronous deep copy"
+    assert call(pageable, pin[1], pin[2], pin[3], pin[4], pin[5], pin[6], pin[7]) == binding.EINVAL
+    assert b"page-locked" in lib.monc_adv_last_error(hd)
+    assert call(pin[0], pin[1], pin[2], pin[3], pin[4], pin[5], pin[6], pageable) == binding.EINVAL
+    # a device pointer is not a host array either
+    dev = torch.zeros(L.shape, dtype=L.torch_dtype, device="cuda")
+    assert call(dev, pin[1], pin[2], pin[3], pin[4], pin[5], pin[6], pin[7]) == binding.EINVAL
+    # overlapping (not merely identical) arrays: an output that starts inside an input
+    big = torch.zeros(2 * int(np.prod(L.shape)), dtype=L.torch_dtype).pin_memory()
+    n = int(np.prod(L.shape))
+    a_in, b_out = big[:n].view(L.shape), big[n // 2 + 2:n // 2 + 2 + n].view(L.shape)
+    assert call(a_in, pin[1], pin[2], pin[3], b_out, pin[5], pin[6], pin[7]) == binding.EINVAL
+    assert b"overlap" in lib.monc_adv_last_error(hd)
+    # nothing is in flight after the refusals: a good call goes through
+    assert call(pin[0], pin[1], pin[2], pin[3], pin[4], pin[5], pin[6], pin[7]) == binding.OK
+    assert lib.monc_adv_step_wait(hd) == binding.OK
     L.close()
