@@ -2,23 +2,29 @@
 """bench.py -- advection grid-points/sec and achieved HBM GB/s on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload config1|config2|config3] [--xchunk X] [--group G]
+                    [--workload config1|config2|config3|config4] [--no-others]
 
-A "step" is one pass of the hot path over one batch of synthetic fields:
-  config1 (default, the configuration BASELINE.json's metric is quoted on):
-      256x256x128 fp64, one fused u/v/w momentum call (SURVEY.md 8(a) a1);
-  config2 / config3: 512x512x256, momentum + 10 batched scalars (a1 + a2),
-      fp64 / fp32 (a4).
-`value` is interior grid points advected per second with inputs resident in
-HBM; `e2e` is the same metric through monc_adv_step_async with PINNED HOST
-buffers (H2D of the fields, kernels, D2H of the tendencies inside the timed
-region).  Prints ONE JSON line (rank 0).
+A "step" is one pass of the whole hot path over one batch of synthetic fields.
+The default workload is BASELINE.json's config 2, the largest single-GPU
+kernel configuration: 512x512x256 fp64, the three momentum fields plus ten
+scalars (every prognostic is advected), the whole step through
+ONE call, monc_adv_tendencies (one fused launch).  `value` is interior grid
+points advected per second over the K timed steps with inputs resident in HBM;
+`e2e` is the same metric through monc_adv_step_async with PINNED HOST buffers
+(H2D of the fields, kernels, D2H of the tendencies inside the timed region,
+SURVEY.md 8(a) a3).  The same line carries a >= 2 s `sustained` record of the
+headline step (the board reaches its power cap within a second), the two
+north_star calls timed kernel by kernel, and compact records of the other
+BASELINE configs (`other_configs`: config1 momentum only, config3 fp32, config4
+the hybrid step from host memory).  Prints ONE JSON line (rank 0).
 
 --impl reference times the CPU oracle (oracle/, fp64, single thread) on the
 same workload: each step is one full oracle pass over the first `--ref-planes`
 x planes of the workload.
 """
 import argparse
+import dataclasses
+import gc
 import json
 import os
 import subprocess
@@ -31,14 +37,25 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
-# algorithmic bytes per interior point: every input read
-# once, every output written once
-BYTES_PER_PT = {"momentum": {"f64": 48, "f32": 24}}
+NOMINAL_GBS = 8000.0  # BASELINE.json: "B200's ~8 TB/s peak", the denominator of the 70 % target
 
 
-def scalar_bytes_per_pt(nq, dtype):
-    es = 8 if dtype == "f64" else 4
-    return 3 * es + 2 * es * nq  # wind once + q in + sq out
+def es_of(dtype):
+    return 8 if dtype == "f64" else 4
+
+
+# algorithmic bytes per interior point: every input read once,
+# every output written once
+def bytes_momentum(dtype):
+    return 6 * es_of(dtype)
+
+
+def bytes_scalars(nq, dtype):
+    return (3 + 2 * nq) * es_of(dtype)  # wind once + q in + sq out
+
+
+def bytes_fused(nq, dtype):
+    return (6 + 2 * nq) * es_of(dtype)  # u, v, w read once for momentum AND scalars
 
 
 def peaks():
@@ -51,8 +68,8 @@ def peaks():
 
 class ClockSampler:
     """SM clock and throttle reasons DURING the timed region: NVML polled from a
-    thread every few ms (the timed region of config1 is milliseconds long, too
-    short for `nvidia-smi -lms`); falls back to the recipe's nvidia-smi line."""
+    thread every few ms (a timed region can be milliseconds long, too short for
+    `nvidia-smi -lms`); falls back to the recipe's nvidia-smi line."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -98,7 +115,7 @@ class ClockSampler:
             self._nvml = nv
             self._thr = threading.Thread(target=poll, daemon=True)
             self._thr.start()
-            return
+            return self
         except Exception:
             self._nvml = None
         try:
@@ -108,6 +125,7 @@ class ClockSampler:
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -144,6 +162,15 @@ def workload_cfg(name):
     return synth.CONFIGS[{"config1": 1, "config2": 2, "config3": 3, "config4": 4}[name]]
 
 
+def config_record(cfg, workload, **extra):
+    """The `config` object: the same keys for our arm and for the reference arm."""
+    nf = 3 + cfg.nq
+    d = {"workload": workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz, "halo": cfg.halo, "nq": cfg.nq,
+         "fields_per_step": nf, "storage_dtype": cfg.dtype}
+    d.update(extra)
+    return d
+
+
 # ncu `dram__bytes_read.sum + dram__bytes_write.sum` per launch of the dominant
 # kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
 # by (workload, kernel family); valid for the library's default launch plan only.
@@ -156,6 +183,23 @@ NCU_TRAFFIC = {
 }
 
 
+def roofline_record(kernel, alg_bytes, ms, launches_per_event, traffic_key, tuned, args):
+    peak, peak_src = peaks()
+    ach = alg_bytes / (ms * 1e-3) / 1e9
+    traffic, traffic_src = args.traffic, "--traffic"
+    if traffic is None:
+        traffic, traffic_src = (None, None) if tuned else NCU_TRAFFIC.get(traffic_key, (None, None))
+        if traffic_src:
+            traffic_src = "committed ncu --set full capture, not re-measured in this run: " + traffic_src
+    return {"bound": "hbm", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": ms, "launches_per_event": launches_per_event,
+            "frac_of_nominal_8TBs": ach / NOMINAL_GBS,
+            # BASELINE.json's "achieved HBM GB/s from ncu": the profiled DRAM bytes of one launch
+            # over this run's measured launch time
+            "ncu_dram_GBs": (traffic / (ms * 1e-3) / 1e9) if traffic else None}
+
+
 # ---------------------------------------------------------------------------
 # reference arm: the CPU oracle as it stands
 # ---------------------------------------------------------------------------
@@ -163,7 +207,6 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import dataclasses
     import oracle
     from paper_2009_12850_b200 import synth
     cfg = workload_cfg(args.workload)
@@ -195,8 +238,10 @@ def run_reference(args):
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz,
-                   "nq": cfg.nq, "halo": cfg.halo},
+        "config": config_record(cfg, args.workload, l2="host memory", parallelism="1 host thread",
+                                step_call="oracle momentum + scalar passes (CPU)", variant="oracle", xchunk=0,
+                                group=0, stages=0, tile_y=0, warps=0, split=0, pdl=False, form=args.form,
+                                launch_plan="none (CPU loops)"),
         "cpu_baseline": {"value": val, "unit": "Gpts/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "Gpts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -206,21 +251,44 @@ def run_reference(args):
 # ---------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
+class Ctx:
+    """torch.distributed plumbing shared by the legs of one run."""
+
+    def __init__(self):
+        import torch
+        self.torch = torch
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            import torch.distributed as dist
+            # NCCL_DEBUG=INFO (set by the caller) shows the communicator over all N ranks
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            self.dist = dist
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, v):
+        if self.world == 1:
+            return float(v)
+        t = self.torch.tensor([v], device="cuda", dtype=self.torch.float64)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
+def make_library(cfg, args):
     from paper_2009_12850_b200 import binding, synth
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    cfg = workload_cfg(args.workload)
     g = synth.grid(cfg.nz)
     L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY,
                         g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=cfg.dtype)
@@ -232,26 +300,62 @@ def run_ours(args):
         L.set_pdl(False)
     if args.form != "flux":
         L.set_form(args.form)
-    tdt = L.torch_dtype
-    # weak scaling: every rank advects its own subdomain of the config's size
-    # ("replicas only" until the halo-exchange row of SURVEY.md 8(f) is built);
-    # rank-keyed seed so ranks do not share data
-    import dataclasses
-    from paper_2009_12850_b200 import dist as pdist
+    return L
+
+
+def is_tuned(args):
+    return any((args.xchunk, args.group, args.stages, args.tile_y, args.warps, args.split, args.variant)) \
+        or args.form != "flux"
+
+
+def host_fields(cfg, rank, cache):
+    """Seeded fp64 host fields of a config; config 3 reuses config 2's (same seeds)."""
+    from paper_2009_12850_b200 import synth
     names = ["u", "v", "w"] + synth.field_names(cfg)
-    if args.halo_exchange:
+    rcfg = cfg if rank == 0 else dataclasses.replace(cfg, seed_cid=1000 + rank)  # ranks do not share data
+    key = (rcfg.seed, cfg.nx, cfg.ny, cfg.nz, cfg.halo, cfg.nq)
+    if key not in cache:
+        cache.clear()
+        cache[key] = [synth.field(rcfg, n) for n in names]
+    return names, cache[key]
+
+
+def timed_loop(ctx, st, fn, nsteps, warm=0):
+    """fn(i) enqueues step i on stream st; device time of nsteps back-to-back steps (ms)."""
+    torch = ctx.torch
+    with torch.cuda.stream(st):
+        for i in range(warm):
+            fn(i)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for i in range(nsteps):
+            fn(warm + i)
+        e1.record(st)
+    return e0, e1
+
+
+def run_device_config(ctx, args, workload, cache, headline):
+    """Configs 1-3: fields resident in HBM.  headline=True: the full record (K timed
+    steps, two-call breakdown, sustained loop, e2e, cpu_baseline); else a compact one."""
+    torch = ctx.torch
+    from paper_2009_12850_b200 import dist as pdist
+    cfg = workload_cfg(workload)
+    L = make_library(cfg, args)
+    tdt = L.torch_dtype
+    names, H = host_fields(cfg, ctx.rank, cache)
+    if args.halo_exchange and headline:
+        from paper_2009_12850_b200 import synth
         # one periodic global domain of world * nx planes, x-slab per rank; the halo
         # swap (PAPER.md:49) runs inside every timed step (SURVEY.md 8(e))
-        gcfg = dataclasses.replace(cfg, nx=world * cfg.nx)
+        gcfg = dataclasses.replace(cfg, nx=ctx.world * cfg.nx)
         H = []
         for n in names:
-            f = pdist.local_from_global(synth.interior_field(gcfg, n), cfg.halo, world, rank)
+            f = pdist.local_from_global(synth.interior_field(gcfg, n), cfg.halo, ctx.world, ctx.rank)
             H.append(pdist.fill_halo_y_periodic(f, cfg.halo).numpy())
-    else:
-        rcfg = cfg if rank == 0 else dataclasses.replace(cfg, seed_cid=1000 + rank)
-        H = [synth.field(rcfg, n) for n in names]
-    nf = len(names)
-    field_bytes = cfg.elems * (8 if cfg.dtype == "f64" else 4)
+    nf, nq = len(names), cfg.nq
+    es = es_of(cfg.dtype)
+    field_bytes = cfg.elems * es
     # rotate between buffer sets so that no step finds its inputs in L2
     nsets = max(2, min(4, int(np.ceil(3 * 126e6 / (2 * nf * field_bytes))) + 1))
     sets = []
@@ -260,109 +364,118 @@ def run_ours(args):
         outs = [torch.zeros(L.shape, device="cuda", dtype=tdt) for _ in names]
         sets.append((ins, outs))
     st = torch.cuda.Stream()
+    swap = args.halo_exchange and headline
 
-    def step(s):
-        ins, outs = sets[s % nsets]
-        if args.halo_exchange:
+    def whole_step(i):  # the step as a user makes it: ONE call when there are scalars
+        ins, outs = sets[i % nsets]
+        if swap:
             pdist.exchange_halo_x(ins, cfg.halo)
-        L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
-        if nf > 3:
-            L.scalars(ins[3:], outs[3:], stream=st)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    with torch.cuda.stream(st):
-        for s in range(args.warmup):
-            step(s)
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    n0 = L.launch_count()
-    # Events are recorded on the launch stream.  Momentum-only workloads: one event
-    # every `grp` launches (an event between two launches costs ~1 us of stream time
-    # and defeats the programmatic dependent launch of back-to-back kernels), so the
-    # mean launch duration is (event span) / grp.  With scalars: one event between
-    # the two kernels of a step as well.
-    split = nf > 3 or args.halo_exchange
-    grp = 1 if split else max(1, min(args.event_every, args.steps))
-    marks = []  # (kind, event)
-    with torch.cuda.stream(st):
-        e0 = torch.cuda.Event(enable_timing=True)
-        e0.record(st)
-        marks.append(("start", e0))
-        for s in range(args.steps):
-            ins, outs = sets[(args.warmup + s) % nsets]
-            if args.halo_exchange:
-                pdist.exchange_halo_x(ins, cfg.halo)
-                e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("swap", e))
+        if nq:
+            L.tendencies(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], ins[3:], outs[3:], stream=st)
+        else:
             L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
-            if split or (s + 1) % grp == 0 or s + 1 == args.steps:
+
+    alg = (bytes_fused(nq, cfg.dtype) if nq else bytes_momentum(cfg.dtype)) * cfg.points
+    steps = args.steps if headline else max(20, min(200, int(0.02 / (alg / 6.0e12))))
+    warm = args.warmup if headline else 3
+
+    # ---- the headline timed region: `steps` whole steps back to back
+    with torch.cuda.stream(st):
+        for i in range(warm):
+            whole_step(i)
+    ctx.barrier()
+    sampler = ClockSampler(ctx.local).start() if ctx.rank == 0 else None
+    n0 = L.launch_count()
+    e0, e1 = timed_loop(ctx, st, whole_step, steps)
+    ctx.barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = L.launch_count() - n0
+    total_ms = ctx.max_over_ranks(e0.elapsed_time(e1))
+    ms_per_step = total_ms / steps
+    value = ctx.world * cfg.points / (ms_per_step * 1e-3) / 1e9
+    plan = L.describe_plan()
+    tsuf = "double" if cfg.dtype == "f64" else "float"
+    fam = "tma" if ("tma_" in plan) else ("march" if "march_" in plan else "generic")
+    if nq and "tma_fused" in plan:
+        kname, tkey = f"tma_scalars<{tsuf}, MOM=1> (fused momentum + scalars)", (workload, "tma_fused")
+    elif nq:
+        kname, tkey = f"{fam}_momentum<{tsuf}> + {fam}_scalars<{tsuf}> (not fused)", (workload, None)
+    else:
+        kname, tkey = f"{fam}_momentum<{tsuf}>", (workload, f"{fam}_momentum")
+    roof = roofline_record(kname, alg, ms_per_step, steps, tkey, is_tuned(args), args)
+    rec = {"value": value, "unit": "Gpts/s", "ms_per_step": ms_per_step, "steps": steps, "warmup": warm,
+           "dtype": cfg.dtype, "gpu_launches": launches, "launch_plan": plan, "roofline": roof, "clocks": clocks,
+           "config": config_record(
+               cfg, workload,
+               l2=f"rotating {nsets} buffer sets ({nsets * 2 * nf * field_bytes / 1e6:.0f} MB) > 126 MB L2",
+               parallelism=("x-slab decomposition, halo swap every step" if swap
+                            else ("replicas only" if ctx.world > 1 else "1 GPU")),
+               step_call="monc_adv_tendencies" if nq else "monc_adv_momentum",
+               variant=args.variant or "auto", xchunk=args.xchunk, group=args.group, stages=args.stages,
+               tile_y=args.tile_y, warps=args.warps, split=args.split, pdl=not args.no_pdl, form=args.form,
+               launch_plan=plan)}
+
+    # ---- sustained: the same step for >= args.sustain_seconds (the board reaches its power
+    # cap within about a second; sw_power_cap is noted, not rejected)
+    if args.sustain_seconds > 0 and not swap:
+        nsus = max(steps, int(np.ceil(args.sustain_seconds * 1e3 / ms_per_step)))
+        ctx.barrier()
+        sm = ClockSampler(ctx.local, period_s=0.02).start() if ctx.rank == 0 else None
+        s0, s1 = timed_loop(ctx, st, whole_step, nsus)
+        ctx.barrier()
+        sclk = sm.stop() if sm else None
+        sms = ctx.max_over_ranks(s0.elapsed_time(s1)) / nsus
+        sg = alg / (sms * 1e-3) / 1e9
+        rec["sustained"] = {"steps": nsus, "seconds": sms * nsus * 1e-3, "ms_per_step": sms,
+                            "value": ctx.world * cfg.points / (sms * 1e-3) / 1e9, "algorithmic_GBs": sg,
+                            "frac": sg / roof["peak"], "frac_of_nominal_8TBs": sg / NOMINAL_GBS, "clocks": sclk}
+    # ---- burst: 20 steps from an idle board, if the headline region was not already that
+    if headline and steps > 40 and not swap:
+        ctx.barrier()
+        time.sleep(2.0)
+        b0, b1 = timed_loop(ctx, st, whole_step, 20, warm=3)
+        ctx.barrier()
+        bms = ctx.max_over_ranks(b0.elapsed_time(b1)) / 20
+        bg = alg / (bms * 1e-3) / 1e9
+        rec["burst"] = {"steps": 20, "ms_per_step": bms, "value": ctx.world * cfg.points / (bms * 1e-3) / 1e9,
+                        "algorithmic_GBs": bg, "frac": bg / roof["peak"], "frac_of_nominal_8TBs": bg / NOMINAL_GBS}
+    if not headline:
+        L.close()
+        del sets
+        gc.collect()
+        torch.cuda.empty_cache()
+        return rec
+
+    # ---- the two north_star calls, kernel by kernel (an event between the two launches)
+    if nq and not swap:
+        tsteps = min(steps, 20)
+        ctx.barrier()
+        time.sleep(1.0)
+        marks = []
+        with torch.cuda.stream(st):
+            for i in range(3):
+                ins, outs = sets[i % nsets]
+                L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
+                L.scalars(ins[3:], outs[3:], stream=st)
+            e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("start", e))
+            for i in range(tsteps):
+                ins, outs = sets[(3 + i) % nsets]
+                L.momentum(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], stream=st)
                 e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("mom", e))
-            if nf > 3:
                 L.scalars(ins[3:], outs[3:], stream=st)
                 e = torch.cuda.Event(enable_timing=True); e.record(st); marks.append(("sca", e))
-    barrier()
-    launches = L.launch_count() - n0
-    plan = L.describe_plan()
-    total_ms = marks[0][1].elapsed_time(marks[-1][1])
-    span = {"swap": 0.0, "mom": 0.0, "sca": 0.0}
-    best = {"swap": 1e30, "mom": 1e30, "sca": 1e30}
-    done = 0
-    for (k0_, a), (k1_, b) in zip(marks[:-1], marks[1:]):
-        ms = a.elapsed_time(b)
-        span[k1_] += ms
-        n_in = 1
-        if k1_ == "mom" and not split:
-            n_in = min(grp, args.steps - done)
-            done += n_in
-        best[k1_] = min(best[k1_], ms / n_in)
-    mom_avg, sca_avg, swap_avg = (span[k] / args.steps for k in ("mom", "sca", "swap"))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * cfg.points * args.steps / (total_ms * 1e-3) / 1e9
-
-    # ---- the same step through monc_adv_tendencies (one fused launch where it fits):
-    # supplementary; `value` above stays the two north_star calls
-    fused = None
-    if nf > 3 and not args.halo_exchange:
-        fsteps = args.steps
-        # the board's power controller averages over ~1 s: let it settle so
-        # this loop starts from the same state as the two-call loop above did
-        barrier()
-        time.sleep(2.0)
-        n1 = L.launch_count()
-        with torch.cuda.stream(st):
-            for s in range(3):
-                ins, outs = sets[s % nsets]
-                L.tendencies(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], ins[3:], outs[3:], stream=st)
-            f0 = torch.cuda.Event(enable_timing=True); f0.record(st)
-            for s in range(fsteps):
-                ins, outs = sets[(3 + s) % nsets]
-                L.tendencies(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], ins[3:], outs[3:], stream=st)
-            f1 = torch.cuda.Event(enable_timing=True); f1.record(st)
-        barrier()
-        ftot = f0.elapsed_time(f1)
-        if world > 1:
-            t = torch.tensor([ftot], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ftot = float(t.item())
-        fms = ftot / fsteps
-        es_ = 8 if cfg.dtype == "f64" else 4
-        fb_ = (6 + 2 * cfg.nq) * es_ * cfg.points  # u, v, w read once; 3 + nq outputs; nq scalars read
-        fused = {"call": "monc_adv_tendencies", "ms_per_step": fms, "value": world * cfg.points / (fms * 1e-3) / 1e9,
-                 "unit": "Gpts/s", "algorithmic_bytes_per_step": fb_, "algorithmic_GBs": fb_ / (fms * 1e-3) / 1e9,
-                 "steps": fsteps, "launches": (L.launch_count() - n1) * fsteps // (fsteps + 3),
-                 "launches_per_step": (L.launch_count() - n1) / (fsteps + 3),
-                 "launch_plan": L.describe_plan()}
-
-    clocks = sampler.stop() if rank == 0 else None
+        ctx.barrier()
+        span = {"mom": 0.0, "sca": 0.0}
+        for (_, a), (k, b) in zip(marks[:-1], marks[1:]):
+            span[k] += a.elapsed_time(b)
+        mom_ms, sca_ms = span["mom"] / tsteps, span["sca"] / tsteps
+        mb, sb = bytes_momentum(cfg.dtype) * cfg.points, bytes_scalars(nq, cfg.dtype) * cfg.points
+        rec["two_call_step"] = {
+            "call": "monc_adv_momentum + monc_adv_scalars", "steps": tsteps, "ms_per_step": mom_ms + sca_ms,
+            "value": ctx.world * cfg.points / ((mom_ms + sca_ms) * 1e-3) / 1e9, "launch_plan": L.describe_plan(),
+            "momentum_ms": mom_ms, "momentum_GBs": mb / (mom_ms * 1e-3) / 1e9,
+            "scalars_ms": sca_ms, "scalars_GBs": sb / (sca_ms * 1e-3) / 1e9,
+            "algorithmic_bytes_per_step": mb + sb}
 
     # ---- end to end through the host-buffer entry point (a3)
     hin = [torch.empty(L.shape, dtype=tdt, pin_memory=True) for _ in names]
@@ -370,7 +483,6 @@ def run_ours(args):
         t_.copy_(torch.from_numpy(a))
     hout = [torch.zeros(L.shape, dtype=tdt, pin_memory=True) for _ in names]
     L.set_chunks(args.chunks)
-
     enqueue_s = [0.0]
 
     def e2e_step():
@@ -379,16 +491,16 @@ def run_ours(args):
         enqueue_s[0] += time.perf_counter() - te  # the host is free from here
         L.step_wait()
 
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e2e_steps = max(1, min(steps, args.e2e_steps))
     for _ in range(2):
         e2e_step()
-    barrier()
+    ctx.barrier()
     enqueue_s[0] = 0.0
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         e2e_step()
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
+    e2e_s = ctx.max_over_ranks(time.perf_counter() - t0)
     enqueue_ms = enqueue_s[0] / e2e_steps * 1e3
     phase = L.step_times_ms()
     # the same step with copies and kernels serialised on one stream: its phases are
@@ -398,122 +510,40 @@ def run_ours(args):
     torch.cuda.synchronize()
     serial = L.step_times_ms()
     L.set_overlap(True)
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    es = 8 if cfg.dtype == "f64" else 4
     plane_b = (cfg.ny + 2 * cfg.halo) * cfg.nz * es
     h2d_b = nf * (cfg.nx + 2) * plane_b
     d2h_b = nf * cfg.points * es
-    e2e_val = world * cfg.points * e2e_steps / e2e_s / 1e9
-
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
-
-    # ---- roofline of the dominant kernel
-    peak, peak_src = peaks()
-    mom_b = BYTES_PER_PT["momentum"][cfg.dtype] * cfg.points
-    sca_b = scalar_bytes_per_pt(cfg.nq, cfg.dtype) * cfg.points if cfg.nq else 0
-    if sca_b and sca_avg > mom_avg:
-        kern, kb, kms = "scalars", sca_b, sca_avg
-    else:
-        kern, kb, kms = "momentum", mom_b, mom_avg
-    fam = {"": "tma", "auto": "tma", "tma": "tma", "march": "march", "generic": "generic"}[args.variant]
-    tsuf = "double" if cfg.dtype == "f64" else "float"
-    achieved = kb / (kms * 1e-3) / 1e9
-    traffic, traffic_src = args.traffic, "--traffic"
-    tuned = any((args.xchunk, args.group, args.stages, args.tile_y, args.warps, args.split)) or args.form != "flux"
-    if traffic is None and not tuned:
-        traffic, traffic_src = NCU_TRAFFIC.get((args.workload, f"{fam}_{kern}"), (None, None))
-    roofline = {"bound": "hbm", "kernel": f"{fam}_{kern}<{tsuf}>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": kb, "avg_launch_ms": kms,
-                "best_launch_ms": best["mom" if kern == "momentum" else "sca"],
-                "launches_per_event": grp if kern == "momentum" else 1,
-                "frac_of_nominal_8TBs": achieved / 8000.0,
-                # BASELINE.json's "achieved HBM GB/s from ncu": the profiled DRAM bytes of
-                # one launch over this run's measured launch time
-                "ncu_dram_GBs": (traffic / (kms * 1e-3) / 1e9) if traffic else None}
-    two_calls = {"value": value, "ms_per_step": total_ms / args.steps, "gpu_launches": launches,
-                 "dominant_kernel_roofline": dict(roofline)}
-    ms_per_step = total_ms / args.steps
-    if fused is not None and not args.two_calls:
-        # the whole step through monc_adv_tendencies is the headline; its kernel the roofline's
-        value, ms_per_step, launches, plan = fused["value"], fused["ms_per_step"], fused["launches"], fused["launch_plan"]
-        if "tma_fused" in plan:
-            ach = fused["algorithmic_bytes_per_step"] / (fused["ms_per_step"] * 1e-3) / 1e9
-            traffic, traffic_src = args.traffic, "--traffic"
-            if traffic is None and not tuned:
-                traffic, traffic_src = NCU_TRAFFIC.get((args.workload, "tma_fused"), (None, None))
-            roofline = {"bound": "hbm", "kernel": f"tma_scalars<{tsuf}, MOM=1> (fused momentum + scalars)",
-                        "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
-                        "traffic_source": traffic_src, "peak_source": peak_src,
-                        "algorithmic_bytes_per_launch": fused["algorithmic_bytes_per_step"],
-                        "avg_launch_ms": fused["ms_per_step"], "launches_per_event": fused["steps"],
-                        "frac_of_nominal_8TBs": ach / 8000.0,
-                        "ncu_dram_GBs": (traffic / (fused["ms_per_step"] * 1e-3) / 1e9) if traffic else None}
-    kernels = {"momentum_ms": mom_avg, "momentum_GBs": mom_b / (mom_avg * 1e-3) / 1e9}
-    if args.halo_exchange:
-        kernels["halo_swap_ms"] = swap_avg
-    if sca_b:
-        kernels.update({"scalars_ms": sca_avg, "scalars_GBs": sca_b / (sca_avg * 1e-3) / 1e9})
-
-    # ---- the oracle beside it: bounded sample on this box's host cores
-    cpu = cpu_baseline(cfg, args)
-
-    out = {
-        "metric": "advection grid-points/sec", "value": value, "unit": "Gpts/s", "n_gpus": world,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
-        "data": "synthetic",
-        "config": {"workload": args.workload, "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz,
-                   "halo": cfg.halo, "nq": cfg.nq, "fields_per_step": nf,
-                   "l2": f"rotating {nsets} buffer sets ({nsets * 2 * nf * field_bytes / 1e6:.0f} MB) > 126 MB L2",
-                   "parallelism": ("x-slab decomposition, halo swap every step" if args.halo_exchange
-                                   else ("replicas only" if world > 1 else "1 GPU")),
-                   "variant": args.variant or "auto", "xchunk": args.xchunk, "group": args.group,
-                   "stages": args.stages, "tile_y": args.tile_y, "warps": args.warps,
-                   "split": args.split, "pdl": not args.no_pdl, "form": args.form,
-                   "step_call": ("monc_adv_tendencies" if (fused is not None and not args.two_calls)
-                                 else ("monc_adv_momentum + monc_adv_scalars" if nf > 3 else "monc_adv_momentum")),
-                   "launch_plan": plan},
-        "roofline": roofline, "kernels": kernels, "fused_step": fused,
-        "two_call_step": two_calls if fused is not None else None, "cpu_baseline": cpu,
-        "e2e": {"value": e2e_val, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b,
-                "d2h_bytes_per_step": d2h_b, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
-                "host_enqueue_ms_per_step": enqueue_ms,
-                "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
-                "phase_ms": phase, "chunks": args.chunks, "serial_phase_ms": serial,
-                "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / phase["total"],
-                "timing": "host wall clock around step_async + step_wait, pinned host buffers"},
-        "gpu_launches": launches, "clocks": clocks,
-    }
-    print(json.dumps(out))
-    if world > 1:
-        dist.destroy_process_group()
+    rec["e2e"] = {"value": ctx.world * cfg.points * e2e_steps / e2e_s / 1e9, "unit": "Gpts/s",
+                  "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b, "steps": e2e_steps,
+                  "ms_per_step": e2e_s / e2e_steps * 1e3, "host_enqueue_ms_per_step": enqueue_ms,
+                  "h2d_GBs": h2d_b / (phase["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (phase["d2h"] * 1e-3) / 1e9,
+                  # the host link alone, one direction at a time (the serialised pass): the
+                  # denominator of the copy/compute overlap (BASELINE.json north_star)
+                  "link_alone_GBs": {"h2d": h2d_b / (serial["h2d"] * 1e-3) / 1e9,
+                                     "d2h": d2h_b / (serial["d2h"] * 1e-3) / 1e9},
+                  "phase_ms": phase, "chunks": args.chunks, "serial_phase_ms": serial,
+                  "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / phase["total"],
+                  "timing": "host wall clock around step_async + step_wait, pinned host buffers"}
+    L.close()
+    del sets, hin, hout
+    gc.collect()
+    torch.cuda.empty_cache()
+    return rec
 
 
 # ---------------------------------------------------------------------------
 # config4: the paper's hybrid asynchronous step as the step
 # ---------------------------------------------------------------------------
-def run_hybrid(args):
+def run_hybrid_config(ctx, args, steps, warmup, with_cpu):
     """1024x1024x160 fp64, 3 momentum + 4 scalars in PINNED HOST memory; a step is
     monc_adv_step_async (8 x-slab chunks H2D -> kernels -> D2H on three streams)
     + monc_adv_step_wait.  Fields are perturbed on the host between steps
     (BASELINE.json configs[4]), outside the timed region: the time of a step is
     the library's device-event span first copy -> last copy, summed over steps."""
-    import torch
-    from paper_2009_12850_b200 import binding, synth
-    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
-        raise SystemExit("config4 is a single-GPU workload (one host link)")
-    torch.cuda.set_device(0)
+    torch = ctx.torch
+    from paper_2009_12850_b200 import synth
     cfg = workload_cfg("config4")
-    g = synth.grid(cfg.nz)
-    L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY,
-                        g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=cfg.dtype)
+    L = make_library(cfg, args)
     L.set_chunks(args.chunks)
     names = ["u", "v", "w"] + synth.field_names(cfg)
     nf = len(names)
@@ -530,13 +560,12 @@ def run_hybrid(args):
         L.step_wait()
         return L.step_times_ms()
 
-    for _ in range(max(1, min(args.warmup, 3))):
+    for _ in range(max(1, min(warmup, 3))):
         step()
-    sampler = ClockSampler(0, period_s=0.05)
-    sampler.start()
+    sampler = ClockSampler(0, period_s=0.05).start()
     n0 = L.launch_count()
     phases = []
-    for s_ in range(args.steps):
+    for s_ in range(steps):
         if not args.no_perturb:
             for n, t in zip(names, hin):
                 synth.perturb(cfg, n, t.numpy(), s_ + 1)
@@ -552,39 +581,143 @@ def run_hybrid(args):
     plane_b = (cfg.ny + 2 * cfg.halo) * cfg.nz * es
     h2d_b = nf * (cfg.nx + 2) * plane_b
     d2h_b = nf * cfg.points * es
-    value = cfg.points * args.steps / (tot_ms * 1e-3) / 1e9
+    value = cfg.points * steps / (tot_ms * 1e-3) / 1e9
     med = {k: float(np.median([p_[k] for p_ in phases])) for k in phases[0]}
+    kb = bytes_fused(cfg.nq, "f64") * cfg.points
     peak, peak_src = peaks()
-    kb = (BYTES_PER_PT["momentum"]["f64"] + scalar_bytes_per_pt(cfg.nq, "f64")) * cfg.points
     ach = kb / (serial["kernels"] * 1e-3) / 1e9
-    e2e = {"value": value, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b,
-           "steps": args.steps, "ms_per_step": tot_ms / args.steps, "chunks": args.chunks,
-           "h2d_GBs": h2d_b / (med["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (med["d2h"] * 1e-3) / 1e9,
-           "link_alone_GBs": {"h2d": h2d_b / (serial["h2d"] * 1e-3) / 1e9,
-                              "d2h": d2h_b / (serial["d2h"] * 1e-3) / 1e9},
-           "phase_ms_median": med, "serial_phase_ms": serial,
-           "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / med["total"]}
-    print(json.dumps({
-        "metric": "advection grid-points/sec", "value": value, "unit": "Gpts/s", "n_gpus": 1,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_ms / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config4", "nx": cfg.nx, "ny": cfg.ny, "nz": cfg.nz, "halo": cfg.halo,
-                   "nq": cfg.nq, "fields_per_step": nf, "chunks": args.chunks,
-                   "perturbed_each_step": not args.no_perturb,
-                   "l2": f"inputs stream from pinned host memory ({h2d_b / 1e9:.2f} GB per step) > 126 MB L2",
-                   "timing": "device events inside the library, first H2D -> last D2H, summed over steps",
-                   "launch_plan": plan},
-        "roofline": {"bound": "hbm", "kernel": "tma_momentum<double> + tma_scalars<double> per chunk",
-                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": kb,
-                     "avg_launch_ms": serial["kernels"],
-                     "note": "kernel time = sum over the 8 chunks, copies not overlapping; the step itself is host-link bound"},
-        "cpu_baseline": cpu_baseline(cfg, args), "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-    }))
+
+    # ---- streaming combine: the host integrates a chunk's source terms as
+    # soon as that chunk has landed, while the later chunks are still on the wire, instead of
+    # waiting for the whole copy.  Integrate = axpy into the host's own copy of su (one field
+    # stands for the model's `step fields`).
+    h = cfg.halo
+    own = np.zeros(L.shape)
+    C = args.chunks
+
+    def integrate(a, b):
+        own[h + a:h + b, h:h + cfg.ny] += 0.5 * hout[0].numpy()[h + a:h + b, h:h + cfg.ny]
+
+    t0 = time.perf_counter()
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+    L.step_wait()
+    t_wait = time.perf_counter() - t0
+    integrate(0, cfg.nx)
+    t_after = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+    for c in range(C):
+        L.step_wait_chunk(c)
+        integrate(*L.step_chunk_range(c))
+    L.step_wait()
+    t_stream = time.perf_counter() - t0
+    # and the on-device combine: the host's source terms go up with the fields,
+    # the kernels add, no separate result buffer -- at the price of the extra H2D
+    L.set_accumulate(True)
+    t0 = time.perf_counter()
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+    L.step_wait()
+    t_devacc = time.perf_counter() - t0
+    L.set_accumulate(False)
+    combine = {"wait_all_then_integrate_ms": t_after * 1e3, "of_which_integrate_ms": (t_after - t_wait) * 1e3,
+               "integrate_as_chunks_land_ms": t_stream * 1e3,
+               "combine_overlap": (t_after - t_stream) / max(t_after - t_wait, 1e-9),
+               "device_accumulate_step_ms": t_devacc * 1e3,
+               "note": "combine_overlap = share of the host's integrate time hidden under the copies still in "
+                       "flight (1 = all of it); device_accumulate uploads the 7 source-term arrays as well"}
+
+    rec = {"value": value, "unit": "Gpts/s", "ms_per_step": tot_ms / steps, "steps": steps, "warmup": warmup,
+           "dtype": "f64", "gpu_launches": launches, "launch_plan": plan, "clocks": clocks,
+           "config": config_record(
+               cfg, "config4", chunks=args.chunks, perturbed_each_step=not args.no_perturb,
+               l2=f"inputs stream from pinned host memory ({h2d_b / 1e9:.2f} GB per step) > 126 MB L2",
+               parallelism="1 GPU", step_call="monc_adv_step_async + monc_adv_step_wait",
+               timing="device events inside the library, first H2D -> last D2H, summed over steps",
+               launch_plan=plan),
+           "roofline": {"bound": "hbm", "kernel": "tma_scalars<double, MOM=1> (fused) per x-slab chunk",
+                        "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                        "peak_source": peak_src, "algorithmic_bytes_per_launch": kb / args.chunks,
+                        "avg_launch_ms": serial["kernels"] / args.chunks, "frac_of_nominal_8TBs": ach / NOMINAL_GBS,
+                        "note": "kernel time = sum over the chunks of the serialised pass (copies not "
+                                "overlapping); the step itself is host-link bound"},
+           "e2e": {"value": value, "unit": "Gpts/s", "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b,
+                   "steps": steps, "ms_per_step": tot_ms / steps, "chunks": args.chunks,
+                   "h2d_GBs": h2d_b / (med["h2d"] * 1e-3) / 1e9, "d2h_GBs": d2h_b / (med["d2h"] * 1e-3) / 1e9,
+                   "link_alone_GBs": {"h2d": h2d_b / (serial["h2d"] * 1e-3) / 1e9,
+                                      "d2h": d2h_b / (serial["d2h"] * 1e-3) / 1e9},
+                   "phase_ms_median": med, "serial_phase_ms": serial,
+                   "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / med["total"],
+                   "streaming_combine": combine}}
+    if with_cpu:
+        rec["cpu_baseline"] = cpu_baseline(cfg, args, "config4")
+    L.close()
+    del hin, hout
+    gc.collect()
+    torch.cuda.empty_cache()
+    return rec
 
 
-def cpu_baseline(cfg, args):
-    import dataclasses
+def compact(rec):
+    """What a sub-record of `other_configs` keeps."""
+    keep = ("value", "unit", "ms_per_step", "steps", "dtype", "gpu_launches", "launch_plan", "clocks",
+            "sustained", "burst")
+    out = {k: rec[k] for k in keep if k in rec}
+    r = rec["roofline"]
+    out["roofline"] = {k: r[k] for k in ("kernel", "achieved", "peak", "frac", "frac_of_nominal_8TBs",
+                                         "algorithmic_bytes_per_launch", "avg_launch_ms") if k in r}
+    out["config"] = {k: rec["config"][k] for k in ("workload", "nx", "ny", "nz", "nq", "storage_dtype", "step_call")}
+    if "e2e" in rec:
+        e = rec["e2e"]
+        out["e2e"] = {k: e[k] for k in ("value", "ms_per_step", "h2d_GBs", "d2h_GBs", "link_alone_GBs",
+                                        "overlap_ratio", "streaming_combine") if k in e}
+    return out
+
+
+def run_ours(args):
+    ctx = Ctx()
+    cache = {}
+    if args.workload == "config4":
+        if ctx.world > 1:
+            raise SystemExit("config4 is a single-GPU workload (one host link)")
+        rec = run_hybrid_config(ctx, args, args.steps, args.warmup, with_cpu=True)
+        cfg = workload_cfg("config4")
+    else:
+        cfg = workload_cfg(args.workload)
+        rec = run_device_config(ctx, args, args.workload, cache, headline=True)
+        if ctx.rank == 0:
+            rec["cpu_baseline"] = cpu_baseline(cfg, args, args.workload)
+    others = {}
+    if not args.no_others and ctx.world == 1 and not args.halo_exchange and not is_tuned(args):
+        for w in ("config3", "config2", "config1", "config4"):  # config 3 first: it reuses config 2's fields
+            if w == args.workload:
+                continue
+            try:
+                if w == "config4":
+                    cache.clear()
+                    others[w] = compact(run_hybrid_config(ctx, args, steps=3, warmup=1, with_cpu=False))
+                else:
+                    others[w] = compact(run_device_config(ctx, args, w, cache, headline=False))
+            except Exception as e:  # a sub-record must not take the headline down with it
+                others[w] = {"error": f"{type(e).__name__}: {e}"}
+    if ctx.rank != 0:
+        ctx.close()
+        return
+    out = {"metric": "advection grid-points/sec", "value": rec["value"], "unit": "Gpts/s", "n_gpus": ctx.world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": rec["ms_per_step"],
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
+           "data": "synthetic", "config": rec["config"], "roofline": rec["roofline"],
+           "cpu_baseline": rec.get("cpu_baseline"), "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
+           "clocks": rec["clocks"]}
+    for k in ("sustained", "burst", "two_call_step"):
+        if k in rec:
+            out[k] = rec[k]
+    if others:
+        out["other_configs"] = others
+    print(json.dumps(out))
+    ctx.close()
+
+
+def cpu_baseline(cfg, args, workload):
     import oracle
     from paper_2009_12850_b200 import synth
     sub = dataclasses.replace(cfg, nx=min(cfg.nx, args.ref_planes))
@@ -617,7 +750,7 @@ def cpu_baseline(cfg, args):
             break
     return {"value": sub.points * reps / dt / 1e9, "unit": "Gpts/s", "cores": 1, "kind": "oracle",
             "sample": f"{reps} oracle passes (fp64, 1 thread) over the first {sub.nx} of {cfg.nx}"
-                      f" x-planes of {args.workload}, {len(names)} fields, {dt:.1f} s",
+                      f" x-planes of {workload}, {len(names)} fields, {dt:.1f} s",
             "all_cores": {"value": sub.points * reps_all / dt_all / 1e9, "unit": "Gpts/s", "cores": nthr,
                           "sample": f"{reps_all} passes of the same sample, {dt_all:.1f} s"},
             "host_cores_available": len(os.sched_getaffinity(0))}
@@ -629,7 +762,11 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config1", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the compact records of the other BASELINE configs")
+    ap.add_argument("--sustain-seconds", type=float, default=2.5,
+                    help="length of the sustained loop of the headline step (0 = skip)")
     ap.add_argument("--xchunk", type=int, default=0)
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--stages", type=int, default=0)
@@ -637,12 +774,8 @@ def main():
     ap.add_argument("--warps", type=int, default=0)
     ap.add_argument("--split", type=int, default=0)
     ap.add_argument("--variant", default="", choices=["", "auto", "generic", "march", "tma"])
-    ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--event-every", type=int, default=10,
-                    help="momentum-only workloads: launches between two timing events")
+    ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-pdl", action="store_true", help="plain stream order between kernels")
-    ap.add_argument("--two-calls", action="store_true",
-                    help="headline = monc_adv_momentum + monc_adv_scalars instead of monc_adv_tendencies")
     ap.add_argument("--form", default="flux", choices=["flux", "pw_skew"],
                     help="flux form (default, BASELINE.json) or the Piacsek-Williams skew form (DESIGN.md R4)")
     ap.add_argument("--ref-planes", type=int, default=64)
@@ -662,8 +795,6 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
-    elif args.workload == "config4":
-        run_hybrid(args)
     else:
         run_ours(args)
 
