@@ -439,6 +439,20 @@ def run_device_config(ctx, args, workload, cache, headline):
         bg = alg / (bms * 1e-3) / 1e9
         rec["burst"] = {"steps": 20, "ms_per_step": bms, "value": ctx.world * cfg.points / (bms * 1e-3) / 1e9,
                         "algorithmic_GBs": bg, "frac": bg / roof["peak"], "frac_of_nominal_8TBs": bg / NOMINAL_GBS}
+    # ---- the paper's work-scaling experiment: the flux arithmetic of every
+    # point evaluated 16 times on the same bytes (ULTIMATE's cost); same results
+    if headline and not swap and not is_tuned(args):
+        ctx.barrier()
+        time.sleep(1.0)
+        L.set_work_scale(16)
+        w0, w1 = timed_loop(ctx, st, whole_step, 10, warm=2)
+        ctx.barrier()
+        L.set_work_scale(1)
+        wms = ctx.max_over_ranks(w0.elapsed_time(w1)) / 10
+        rec["work_scale_16"] = {"steps": 10, "ms_per_step": wms, "ratio_to_x1": wms / ms_per_step,
+                                "value": ctx.world * cfg.points / (wms * 1e-3) / 1e9,
+                                "note": "kernel time with 16 x the arithmetic per byte; the hybrid step through the "
+                                        "host link is timed at x16 in other_configs.config4 (PAPER.md:109)"}
     if not headline:
         L.close()
         del sets
@@ -619,6 +633,14 @@ def run_hybrid_config(ctx, args, steps, warmup, with_cpu):
     L.step_wait()
     t_devacc = time.perf_counter() - t0
     L.set_accumulate(False)
+    # the paper's x16 work-scaled run: "the GPU times look very similar"
+    L.set_work_scale(16)
+    t0 = time.perf_counter()
+    L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+    L.step_wait()
+    t_x16 = time.perf_counter() - t0
+    x16 = L.step_times_ms()
+    L.set_work_scale(1)
     combine = {"wait_all_then_integrate_ms": t_after * 1e3, "of_which_integrate_ms": (t_after - t_wait) * 1e3,
                "integrate_as_chunks_land_ms": t_stream * 1e3,
                "combine_overlap": (t_after - t_stream) / max(t_after - t_wait, 1e-9),
@@ -647,7 +669,10 @@ def run_hybrid_config(ctx, args, steps, warmup, with_cpu):
                                       "d2h": d2h_b / (serial["d2h"] * 1e-3) / 1e9},
                    "phase_ms_median": med, "serial_phase_ms": serial,
                    "overlap_ratio": (serial["h2d"] + serial["kernels"] + serial["d2h"]) / med["total"],
-                   "streaming_combine": combine}}
+                   "streaming_combine": combine,
+                   "work_scale_16": {"step_ms": x16["total"], "kernels_ms": x16["kernels"], "wall_ms": t_x16 * 1e3,
+                                     "step_ratio_to_x1": x16["total"] / med["total"],
+                                     "kernels_ratio_to_x1": x16["kernels"] / med["kernels"]}}}
     if with_cpu:
         rec["cpu_baseline"] = cpu_baseline(cfg, args, "config4")
     L.close()
@@ -669,7 +694,7 @@ def compact(rec):
     if "e2e" in rec:
         e = rec["e2e"]
         out["e2e"] = {k: e[k] for k in ("value", "ms_per_step", "h2d_GBs", "d2h_GBs", "link_alone_GBs",
-                                        "overlap_ratio", "streaming_combine") if k in e}
+                                        "overlap_ratio", "streaming_combine", "work_scale_16") if k in e}
     return out
 
 
@@ -708,7 +733,7 @@ def run_ours(args):
            "data": "synthetic", "config": rec["config"], "roofline": rec["roofline"],
            "cpu_baseline": rec.get("cpu_baseline"), "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
            "clocks": rec["clocks"]}
-    for k in ("sustained", "burst", "two_call_step"):
+    for k in ("sustained", "burst", "two_call_step", "work_scale_16"):
         if k in rec:
             out[k] = rec[k]
     if others:

@@ -191,6 +191,14 @@ int monc_adv_set_form(monc_adv_t h, int form);
 /* 0 (default): tendencies overwritten.  1: added into the output buffers (device
  * arrays of momentum / scalars / tendencies; host arrays of step_async, see there). */
 int monc_adv_set_accumulate(monc_adv_t h, int on);
+/* The paper's work-scaling experiment ("we have also scaled the workload
+ * of the PW advection scheme to match that of the ULTIMATE scheme ... the GPU times
+ * look very similar"; PAPER.md:97 puts ULTIMATE at about 16 x PW): every kernel
+ * evaluates the flux arithmetic of a point n times (1 <= n <= 64, default 1) on the
+ * same bytes.  Results are identical to n = 1.  Needs the flux form, overwrite mode
+ * and the default (TMA) kernels: EINVAL otherwise, and for shapes whose nz is not a
+ * multiple of 16 bytes / sizeof(dtype) the compute calls return EINVAL while n > 1. */
+int monc_adv_set_work_scale(monc_adv_t h, int n);
 /* 1 (default): monc_adv_tendencies and monc_adv_step_async use the fused
  * momentum + scalars launch where it fits.  0: always two launches. */
 int monc_adv_set_fuse(monc_adv_t h, int on);

@@ -17,6 +17,7 @@ import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmonc_adv.so")
+LIB_PATH_CHECKED = os.path.join(HERE, "libmonc_adv_checked.so")  # -DMONC_ADV_CHECKED=1 (tests/test_gpu_checked.py)
 
 F64, F32 = 0, 1
 FORM_FLUX, FORM_PW_SKEW = 0, 1
@@ -31,7 +32,7 @@ SYMBOLS = [
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
-    "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version",
+    "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version", "monc_adv_set_work_scale",
 ]
 
 
@@ -42,6 +43,16 @@ class MoncAdvError(RuntimeError):
 
 
 _lib = None
+_libs = {}
+_path = LIB_PATH
+
+
+def select_build(checked: bool) -> None:
+    """Handles created from now on come from the checked build (poisoned ring slots,
+    jittered schedule; same ABI, same results) or from the normal one."""
+    global _lib, _path
+    _path = LIB_PATH_CHECKED if checked else LIB_PATH
+    _lib = None
 
 
 def load():
@@ -49,10 +60,13 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        raise MoncAdvError(ECUDA, f"{LIB_PATH} not built: run `python -m paper_2009_12850_b200.build`"
+    if _path in _libs:
+        _lib = _libs[_path]
+        return _lib
+    if not os.path.exists(_path):
+        raise MoncAdvError(ECUDA, f"{_path} not built: run `python -m paper_2009_12850_b200.build`"
                            " (there is no CPU fallback)")
-    lib = C.CDLL(LIB_PATH)
+    lib = C.CDLL(_path)
     vp, dp, ci = C.c_void_p, C.POINTER(C.c_double), C.c_int
     lib.monc_adv_create.argtypes = [C.POINTER(vp), ci, ci, ci, ci, C.c_double, C.c_double] + [dp] * 8 + [ci]
     lib.monc_adv_create.restype = ci
@@ -79,7 +93,7 @@ def load():
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
                  "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
-                 "monc_adv_set_fuse"):
+                 "monc_adv_set_fuse", "monc_adv_set_work_scale"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -94,6 +108,7 @@ def load():
     lib.monc_adv_last_error.restype = C.c_char_p
     lib.monc_adv_version.argtypes = []
     lib.monc_adv_version.restype = C.c_char_p
+    _libs[_path] = lib
     _lib = lib
     return lib
 
@@ -251,6 +266,9 @@ class MoncAdv:
 
     def set_pdl(self, on):
         self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
+
+    def set_work_scale(self, n):
+        self._check(self._lib.monc_adv_set_work_scale(self._h, int(n)))
 
     def set_fuse(self, on):
         self._check(self._lib.monc_adv_set_fuse(self._h, int(bool(on))))

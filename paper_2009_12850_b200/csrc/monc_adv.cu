@@ -62,7 +62,7 @@ struct monc_adv_s {
   void *d_tz[4] = {nullptr, nullptr, nullptr, nullptr};  // tzc1, tzc2, tzd1, tzd2 (dtype)
   std::vector<double> tz_host[4];                        // as stored on the device
   const void *wind[3] = {nullptr, nullptr, nullptr};
-  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1, fuse = 1;
+  int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1, fuse = 1, work = 1;
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
@@ -150,6 +150,7 @@ KParams<T> make_params(monc_adv_t h, int ia, int ib) {
   p.accumulate = h->accumulate;
   p.skew = h->form == MONC_ADV_FORM_PW_SKEW;
   p.prefetch = h->prefetch < 0 ? 0 : (h->prefetch == 0 ? kDefaultPrefetch : h->prefetch);
+  p.work = h->work;
   p.cx = (T)(1.0 / (4.0 * h->dx));
   p.cy = (T)(1.0 / (4.0 * h->dy));
   p.tzc1 = (const T *)h->d_tz[0]; p.tzc2 = (const T *)h->d_tz[1];
@@ -183,17 +184,17 @@ int pick_xchunk(monc_adv_t h, int nplanes, int blocks_per_plane, int resident_pe
 // (20 SMs on 16 SMs' worth of bandwidth: 1.27 x at 148 blocks).  Several waves of
 // short blocks are balanced dynamically: about 1.12 block-times per 148 blocks,
 // plus half a block-time for the ragged end.  A single wave that leaves SMs idle
-// is charged for them (0.95 x SMs / blocks): under the board's power cap the SM
+// is charged for them (0.93 x SMs / blocks): under the board's power cap the SM
 // clock drops and the per-SM rate, not DRAM, bounds the launch (config 2 momentum,
 // 128 blocks x 512 planes against 1024 x 64: 4 % faster in a burst, 6 % slower
 // sustained).
 double launch_rounds(long blocks, int sm_count) {
   const long full_rate = std::max(1L, (long)sm_count * 128 / 148);
-  const double idle = 0.95 * (double)sm_count / (double)std::max(1L, blocks);
-  if (blocks <= full_rate) return std::max(1.0, idle);
-  if (blocks <= sm_count)
-    return std::max(idle, 1.0 + 0.27 * (double)(blocks - full_rate) / (double)(sm_count - full_rate));
-  if (blocks < 2L * sm_count) return 1.12 + 1.0;  // one full wave and a partial one, each a whole block-time
+  auto gpc_wave = [&](long b) {
+    return b <= full_rate ? 1.0 : 1.0 + 0.27 * (double)(b - full_rate) / (double)(sm_count - full_rate);
+  };
+  if (blocks <= sm_count) return std::max(gpc_wave(blocks), 0.93 * (double)sm_count / (double)std::max(1L, blocks));
+  if (blocks < 2L * sm_count) return 1.12 + gpc_wave(blocks - sm_count);  // a full wave, then a static partial one
   return 1.12 * (double)blocks / (double)sm_count + 0.5;
 }
 
@@ -290,6 +291,7 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
   if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia);
   if (h->variant == 3 && !pl.ok)
     return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
+  if (h->work > 1 && !pl.ok) return fail(h, MONC_ADV_EINVAL, "momentum: work scaling needs the TMA kernels");
   if (pl.ok) {
     p.xc = pl.xc;
     dim3 grid(pl.tiles, pl.nchunks);
@@ -299,8 +301,9 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
       return MONC_ADV_OK;
     };
     const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
-    const int rc = h->accumulate ? (skew ? go(tma_momentum<T, true, true>) : go(tma_momentum<T, true, false>))
-                                 : (skew ? go(tma_momentum<T, false, true>) : go(tma_momentum<T, false, false>));
+    const int rc = h->work > 1 ? go(tma_momentum<T, false, false, true>)  // checked by work_scale_ok: flux, overwrite
+                   : h->accumulate ? (skew ? go(tma_momentum<T, true, true>) : go(tma_momentum<T, true, false>))
+                                   : (skew ? go(tma_momentum<T, false, true>) : go(tma_momentum<T, false, false>));
     if (rc != MONC_ADV_OK) return rc;
     char b[160];
     snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d threads=%d smem=%zu", pl.ty,
@@ -484,13 +487,13 @@ const TensorMaps *field_maps(monc_adv_t h, const T *u, const T *v, const T *w, c
   return &slot->maps;
 }
 
-template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false>
 int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
                          const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM>));
+  CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>));
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
                 (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz));
   return MONC_ADV_OK;
 }
@@ -499,6 +502,8 @@ template <typename T, int GW, bool MOM>
 int launch_tma_scalars_m(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
                          const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
   const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
+  if (h->work > 1)  // checked by work_scale_ok: flux form, overwrite
+    return launch_tma_scalars_k<T, GW, false, false, MOM, true>(h, p, maps, outs, mo, nq, pl, st);
   if (h->accumulate)
     return skew ? launch_tma_scalars_k<T, GW, true, true, MOM>(h, p, maps, outs, mo, nq, pl, st)
                 : launch_tma_scalars_k<T, GW, true, false, MOM>(h, p, maps, outs, mo, nq, pl, st);
@@ -582,6 +587,7 @@ int launch_scalars(monc_adv_t h, const T *u, const T *v, const T *w, const void 
   }
   if (h->variant == 3)
     return fail(h, MONC_ADV_EINVAL, "scalars: TMA variant does not fit this nz / form");
+  if (h->work > 1) return fail(h, MONC_ADV_EINVAL, "scalars: work scaling needs the TMA kernels");
   if (use_march<T>(h)) {
     int G = h->group > 0 ? std::min(h->group, 5) : (nq >= 5 ? 5 : nq);
     G = std::min(G, nq);
@@ -1098,13 +1104,24 @@ int monc_adv_set_form(monc_adv_t h, int form) {
   if (!h) return MONC_ADV_EINVAL;
   if (form != MONC_ADV_FORM_FLUX && form != MONC_ADV_FORM_PW_SKEW)
     return fail(h, MONC_ADV_EINVAL, "set_form: unknown form");
+  if (form != MONC_ADV_FORM_FLUX && h->work > 1) return fail(h, MONC_ADV_EINVAL, "set_form: work scaling is on (flux form only)");
   h->form = form;
   return MONC_ADV_OK;
 }
 
 int monc_adv_set_accumulate(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
+  if (on && h->work > 1) return fail(h, MONC_ADV_EINVAL, "set_accumulate: work scaling is on (overwrite mode only)");
   h->accumulate = on ? 1 : 0;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_work_scale(monc_adv_t h, int n) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (n < 1 || n > 64) return fail(h, MONC_ADV_EINVAL, "set_work_scale: need 1 <= n <= 64");
+  if (n > 1 && (h->form != MONC_ADV_FORM_FLUX || h->accumulate || (h->variant != 0 && h->variant != 3)))
+    return fail(h, MONC_ADV_EINVAL, "set_work_scale: needs the flux form, overwrite mode and the TMA kernels");
+  h->work = n;
   return MONC_ADV_OK;
 }
 
@@ -1117,6 +1134,8 @@ int monc_adv_set_pdl(monc_adv_t h, int on) {
 int monc_adv_set_variant(monc_adv_t h, int variant) {
   if (!h) return MONC_ADV_EINVAL;
   if (variant < 0 || variant > 3) return fail(h, MONC_ADV_EINVAL, "set_variant: 0..3");
+  if (h->work > 1 && variant != 0 && variant != 3)
+    return fail(h, MONC_ADV_EINVAL, "set_variant: work scaling is on (TMA kernels only)");
   if (variant >= 2) {
     const int nk = h->dtype == MONC_ADV_F64 ? 2 : 4;
     if (h->nz % nk != 0) return fail(h, MONC_ADV_EINVAL, "set_variant: marching kernels need nz % (16/sizeof(dtype)) == 0");
@@ -1164,6 +1183,12 @@ const char *monc_adv_last_error(monc_adv_t h) {
   return h ? h->err.c_str() : g_create_error.c_str();
 }
 
-const char *monc_adv_version(void) { return "monc-adv-b200 0.1 (sm_100a)"; }
+const char *monc_adv_version(void) {
+#if MONC_ADV_CHECKED
+  return "monc-adv-b200 0.2 (sm_100a, checked build: poisoned ring slots, jittered schedule)";
+#else
+  return "monc-adv-b200 0.2 (sm_100a)";
+#endif
+}
 
 }  // extern "C"

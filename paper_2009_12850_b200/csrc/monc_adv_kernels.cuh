@@ -45,6 +45,7 @@ struct KParams {
   int accumulate;   // 0: overwrite, 1: add into outputs
   int skew;         // generic kernels only: PW skew form
   int prefetch;     // march kernels: L2 prefetch distance in planes (0 = off)
+  int work;         // TMA kernels, WS instantiations: evaluations of the flux arithmetic per point
   T cx, cy;         // 1/(4dx), 1/(4dy)
   const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz; tzc2[nz-1] = 0
 };
@@ -109,6 +110,16 @@ __device__ __forceinline__ Vec<T> ld_or_zero(const T *p, bool act) {
 }
 
 constexpr unsigned kFull = 0xffffffffu;
+
+// the compiler must assume x changed: re-evaluations of the same arithmetic (the
+// work-scaling experiment of PAPER.md:109) are neither merged nor hoisted
+__device__ __forceinline__ void opaque(double &x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void opaque(float &x) { asm volatile("" : "+f"(x)); }
+template <typename T>
+__device__ __forceinline__ void opaque(Vec<T> &a) {
+#pragma unroll
+  for (int e = 0; e < VecOf<T>::NK; ++e) opaque(a.v[e]);
+}
 
 __device__ __forceinline__ void prefetch_l2(const void *p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));

@@ -72,6 +72,41 @@ __device__ __forceinline__ void pdl_launch_dependents() {
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------
+// Checked build (-DMONC_ADV_CHECKED=1 -> libmonc_adv_checked.so; tests/test_gpu_checked.py).
+// compute-sanitizer is closed on the pool this library is developed on, so the
+// ring protocol is shaken out from the inside instead:
+//   poison  every ring slot is filled with NaN before each TMA refill (and the whole
+//           ring at kernel start): a value read from a slot location the copy did not
+//           write, or from a slot released too early and already poisoned for the
+//           next plane, reaches an output as NaN and fails the parity tests
+//           (initcheck / racecheck on the ring, by construction of the data);
+//   jitter  every warp sleeps a pseudo-random 0..2 us before it reads a slot, before
+//           it releases one and (producers) before a refill, so that orderings the
+//           undisturbed schedule never produces are exercised.
+// Results are bitwise those of the normal build (same arithmetic).
+// ---------------------------------------------------------------------------
+#ifndef MONC_ADV_CHECKED
+#define MONC_ADV_CHECKED 0
+#endif
+__device__ __forceinline__ void chk_jitter(const unsigned salt) {
+#if MONC_ADV_CHECKED
+  unsigned x = (unsigned)clock64() * 2654435761u + salt * 40503u + blockIdx.x * 9176u + (threadIdx.x >> 5) * 7919u;
+  x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+  if (x & 1u) __nanosleep(x & 2047u);
+#endif
+}
+// NaN-fill `bytes` bytes of shared memory at `dst` with the `nthr` threads that call it
+// (thread `tid` of them), then order the generic-proxy stores before later async-proxy
+// (TMA) writes to the same locations
+__device__ __forceinline__ void chk_poison(const uint32_t dst, const uint32_t bytes, const int tid, const int nthr) {
+#if MONC_ADV_CHECKED
+  for (uint32_t o = 8u * tid; o + 8u <= bytes; o += 8u * nthr)
+    asm volatile("st.shared.b64 [%0], %1;" ::"r"(dst + o), "l"(0x7ff8dead7ff8deadull) : "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+#endif
+}
+
+// ---------------------------------------------------------------------------
 // Shared-memory loads by 32-bit shared-window address with a compile-time byte
 // offset folded into the instruction ([R + imm]): the consumers' address
 // arithmetic is then a handful of 32-bit adds per plane.
@@ -152,6 +187,7 @@ template <typename T>
 struct MarchArgs {
   uint32_t a0, fb, sbytes, rsb, bar0;
   int nstages, nsteps, lane;
+  int work;  // WS: evaluations of the arithmetic per step (results identical)
   bool act, bot_edge;
   bool first_level, last_level;  // element 0 is level K = 1 (no tendency) / element NK-1 is level K = nz (sw = 0)
   T *su, *sv, *sw;            // output arrays (kernel parameters: re-read from the constant bank, not kept in registers)
@@ -160,7 +196,7 @@ struct MarchArgs {
   Vec<T> c1, c2, d1, d2;
 };
 
-template <typename T, bool ACC, bool SKEW, typename AfterRelease>
+template <typename T, bool ACC, bool SKEW, bool WS, typename AfterRelease>
 __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelease &&after_release) {
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
@@ -190,6 +226,7 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
   bool first = true;
   auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
     mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
+    chk_jitter(1);
     const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
     const Vec<T> uS = lds_at<0>(pC - rsb, tag), uN = lds_at<0>(pC + rsb, tag);
     const Vec<T> vN = lds_at<0>(pCv + rsb, tag);
@@ -216,9 +253,22 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
       }
     }
     Vec<T> ou, ov, ow;
-    momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, m.c1,
-                            m.c2, m.d1, m.d2, m.cx, m.cy, lane, ou, ov, ow);
+    if constexpr (WS) {
+      // the paper's work-scaling experiment: the same arithmetic m.work
+      // times on the same bytes; every evaluation gives the same result
+#pragma unroll 1
+      for (int r = 0; r < m.work; ++r) {
+        PlaneRegs<T> &Rc = const_cast<PlaneRegs<T> &>(RC);  // the registers themselves, values unchanged
+        opaque(Rc.u); opaque(Rc.v); opaque(Rc.vs); opaque(Rc.w);
+        momentum_faces<T, SKEW>(Rc, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz,
+                                m.c1, m.c2, m.d1, m.d2, m.cx, m.cy, lane, ou, ov, ow);
+      }
+    } else {
+      momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, m.c1,
+                              m.c2, m.d1, m.d2, m.cx, m.cy, lane, ou, ov, ow);
+    }
     // this warp is done with the centre plane's slot
+    chk_jitter(2);
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
     if (!first) {
@@ -267,7 +317,7 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
 // dynamic shared memory: nstages * 3 * (ty+2) * nz elements, then 2*nstages
 // mbarriers.
 // ---------------------------------------------------------------------------
-template <typename T, bool ACC, bool SKEW>
+template <typename T, bool ACC, bool SKEW, bool WS = false>
 __global__ void __launch_bounds__(kTmaThreads, 1)
 tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__restrict__ u,
              const T *__restrict__ v, const T *__restrict__ w, T *__restrict__ su,
@@ -296,6 +346,7 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  chk_poison(smem_u32(smem_raw), (uint32_t)(nstages * stagesz * SZ), threadIdx.x, blockDim.x);
   __syncthreads();
 
   pdl_launch_dependents();
@@ -338,6 +389,7 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   m.a0 = t0 + (uint32_t)(((col + 1) * nz + k0) * SZ);  // u(column, k0) in stage 0
   m.fb = fb; m.sbytes = sb; m.rsb = (uint32_t)(nz * SZ); m.bar0 = bar0;
   m.nstages = nstages; m.nsteps = nsteps; m.lane = lane;
+  m.work = p.work;
   m.bot_edge = m.act && lane == 0 && zc > 0;
   m.first_level = k0 == 0;
   m.last_level = k0 + NK == nz;
@@ -345,10 +397,12 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   m.su = su; m.sv = sv; m.sw = sw;
   m.plane = p.plane;
   m.cx = p.cx; m.cy = p.cy;
-  momentum_march<T, ACC, SKEW>(m, [&]() {
+  momentum_march<T, ACC, SKEW, WS>(m, [&]() {
     if (producer && to_issue > 0) {
       // slot of plane i-1: every warp released it during the previous step
       mbar_wait(bar0 + 8 * (nstages + s_next), par_next);
+      chk_jitter(3);
+      chk_poison(t0 + (uint32_t)s_next * sb, sb, 0, 1);
       issue_plane();
       if (s_next == 0) par_next ^= 1;
     }
@@ -434,10 +488,10 @@ constexpr int kRowBytes = 34 * 16;  // 32 vectors of the tile + one vector of z 
 
 // The scalar role of one warp: GW scalars (mycnt of them live when !FULL) of one
 // column chunk over the block's planes.
-template <typename T, int GW, bool ACC, bool SKEW, bool FULL>
+template <typename T, int GW, bool ACC, bool SKEW, bool FULL, bool WS>
 __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t fb, const uint32_t sbytes,
                                              const uint32_t q0off, const uint32_t bar0, const int nstages,
-                                             const int nplanes, const int mycnt, const int lane,
+                                             const int nplanes, const int mycnt, const int work, const int lane,
                                              const bool act, const bool bot_edge, const int keep_first,
                                              T *const *__restrict__ sqp, const long long c0,
                                              const long long plane, const Vec<T> &c1, const Vec<T> &c2,
@@ -465,6 +519,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
   auto step = [&](auto store_tag, const Vec<T> (&QP)[GW], Vec<T> (&QN)[GW], const Vec<T> &ux, Vec<T> &un) {
     constexpr bool STORE = decltype(store_tag)::value;
     mbar_wait(bar0 + 8 * st, par);  // the next plane has landed
+    chk_jitter(4);
     const uint32_t pV = pA + fb, pW = pV + fb;
     Vec<T> vs = lds_at<-RSB>(pV, tag), vn = lds_at<0>(pV, tag);
     Vec<T> wt = lds_at<0>(pW, tag);
@@ -483,42 +538,58 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
         QN[s] = lds_at<0>(pQ, tag);
         const Vec<T> &q = QN[s];
         const Vec<T> qS = lds_at<-RSB>(pQ, tag), qN = lds_at<RSB>(pQ, tag);
-        const Vec<T> qU = up_with(q, lds1_at<UP>(pQ, tag));
+        const T qtop = lds1_at<UP>(pQ, tag);  // the level above the thread's last
         // the level below the thread's first: lane 0 reads it, the others get it by shuffle
         const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
-        Vec<T> o;
-        if (SKEW) {
-          // Piacsek-Williams skew form (R4): the advected parenthesis holds the
-          // far value only, so each face contributes the neighbour's value times the
-          // (scaled) advecting velocity
-          const T prv = __shfl_up_sync(kFull, q.v[NK - 1], 1);
-          const Vec<T> qD = down_with(q, lane == 0 ? qb : prv);
+        Vec<T> o, can;
+        // o: the previous plane's tendency, complete; can: this plane's A.  qc is the centre
+        // vector the arithmetic reads (q itself, or an opaque copy when the work is repeated)
+        auto evaluate = [&](const Vec<T> &qc) {
+          const Vec<T> qU = up_with(qc, qtop);
+          if (SKEW) {
+            // Piacsek-Williams skew form (R4): the advected parenthesis holds the
+            // far value only, so each face contributes the neighbour's value times the
+            // (scaled) advecting velocity
+            const T prv = __shfl_up_sync(kFull, qc.v[NK - 1], 1);
+            const Vec<T> qD = down_with(qc, lane == 0 ? qb : prv);
 #pragma unroll
-          for (int e = 0; e < NK; ++e) {
-            T y = vn.v[e] * qN.v[e];
-            y = vs.v[e] * qS.v[e] - y;
-            y = wl.v[e] * qD.v[e] + y;
-            y = y - wt.v[e] * qU.v[e];
-            o.v[e] = CA[s].v[e] - ux.v[e] * q.v[e];
-            CA[s].v[e] = y + ux.v[e] * QP[s].v[e];
+            for (int e = 0; e < NK; ++e) {
+              T y = vn.v[e] * qN.v[e];
+              y = vs.v[e] * qS.v[e] - y;
+              y = wl.v[e] * qD.v[e] + y;
+              y = y - wt.v[e] * qU.v[e];
+              o.v[e] = CA[s].v[e] - ux.v[e] * qc.v[e];
+              can.v[e] = y + ux.v[e] * QP[s].v[e];
+            }
+          } else {
+            Vec<T> g;
+#pragma unroll
+            for (int e = 0; e < NK; ++e) g.v[e] = qc.v[e] + qU.v[e];
+            const T prv = __shfl_up_sync(kFull, g.v[NK - 1], 1);
+            const Vec<T> gD = down_with(g, lane == 0 ? qb + qc.v[0] : prv);
+#pragma unroll
+            for (int e = 0; e < NK; ++e) {
+              T y = vn.v[e] * (qc.v[e] + qN.v[e]);
+              y = vs.v[e] * (qS.v[e] + qc.v[e]) - y;
+              y = wl.v[e] * gD.v[e] + y;
+              y = y - wt.v[e] * g.v[e];  // P: the y and z flux differences of this plane
+              const T sx = QP[s].v[e] + qc.v[e];
+              o.v[e] = CA[s].v[e] - ux.v[e] * sx;  // minus the flux through the face between the two planes
+              can.v[e] = y + ux.v[e] * sx;
+            }
+          }
+        };
+        if constexpr (WS) {
+          // the same arithmetic `work` times on the same bytes, same result
+#pragma unroll 1
+          for (int r = 0; r < work; ++r) {
+            opaque(QN[s]);  // the registers themselves, values unchanged
+            evaluate(QN[s]);
           }
         } else {
-          Vec<T> g;
-#pragma unroll
-          for (int e = 0; e < NK; ++e) g.v[e] = q.v[e] + qU.v[e];
-          const T prv = __shfl_up_sync(kFull, g.v[NK - 1], 1);
-          const Vec<T> gD = down_with(g, lane == 0 ? qb + q.v[0] : prv);
-#pragma unroll
-          for (int e = 0; e < NK; ++e) {
-            T y = vn.v[e] * (q.v[e] + qN.v[e]);
-            y = vs.v[e] * (qS.v[e] + q.v[e]) - y;
-            y = wl.v[e] * gD.v[e] + y;
-            y = y - wt.v[e] * g.v[e];  // P: the y and z flux differences of this plane
-            const T sx = QP[s].v[e] + q.v[e];
-            o.v[e] = CA[s].v[e] - ux.v[e] * sx;  // minus the flux through the face between the two planes
-            CA[s].v[e] = y + ux.v[e] * sx;
-          }
+          evaluate(q);
         }
+        CA[s] = can;
         if (STORE && act) {  // sq of the previous plane is complete
           o.v[0] = keep_if(o.v[0], keep_first);
           T *sq = sqp[s] + c;  // pointer table lives in the constant bank
@@ -533,6 +604,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
       }
     }
     // this warp is done with the slot
+    chk_jitter(5);
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
     if (STORE) c += plane;
@@ -553,7 +625,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
   }
 }
 
-template <typename T, int GW, bool ACC, bool SKEW, bool MOM>
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const MomPtrs<T> mo, const int nq, const int ngroups, const int gb, const int ty,
@@ -597,6 +669,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  chk_poison(t0, (uint32_t)(nstages * stagesz * SZ), threadIdx.x, blockDim.x);
   __syncthreads();
 
   pdl_launch_dependents();
@@ -613,6 +686,8 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
 #pragma unroll 1
     for (int n = 0; n < nplanes; ++n) {
       mbar_wait(bar0 + 8 * (nstages + s), par);  // every consumer warp released the slot
+      chk_jitter(6);
+      if (n >= nstages) chk_poison(t0 + (uint32_t)(s * stagesz * SZ), (uint32_t)(stagesz * SZ), lane, 32);
       const uint32_t full = bar0 + 8 * s;
       if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
       __syncwarp();
@@ -644,6 +719,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     m.d1 = ld_vec(p.tzd1 + k0); m.d2 = ld_vec(p.tzd2 + k0);
     m.a0 = a0; m.fb = fb; m.sbytes = sbytes; m.rsb = (uint32_t)kRowBytes; m.bar0 = bar0;
     m.nstages = nstages; m.nsteps = nplanes - 1; m.lane = lane;
+    m.work = p.work;
     m.act = act; m.bot_edge = bot_edge;
     m.first_level = k0 == 0;
     m.last_level = k0 + NK == nz;
@@ -651,7 +727,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     m.c0 = c0; m.plane = p.plane;
     m.cx = p.cx; m.cy = p.cy;
     pdl_wait();
-    momentum_march<T, ACC, SKEW>(m, []() {});
+    momentum_march<T, ACC, SKEW, WS>(m, []() {});
     return;
   }
   if (sp >= slive) return;
@@ -665,11 +741,11 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   T *const *sqp = outs.sq + (s0 + sb);
   pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
   if (mycnt == GW)
-    scalar_march<T, GW, ACC, SKEW, true>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, lane, act,
-                                         bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, true, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, lane,
+                                             act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
   else
-    scalar_march<T, GW, ACC, SKEW, false>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, lane, act,
-                                          bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, false, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, lane,
+                                              act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
 }
 
 }  // namespace monc

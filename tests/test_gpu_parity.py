@@ -469,3 +469,53 @@ def test_tendencies_errors():
     L.scalars(d[3:], o[3:])  # the wind is bound by tendencies
     torch.cuda.synchronize()
     L.close()
+
+
+# ---------------------------------------------------------------------------
+# the paper's work-scaling experiment: the flux
+# arithmetic evaluated n times on the same bytes gives the result of n = 1, bitwise
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_work_scale_is_the_identity_bitwise(dtype):
+    cfg = gc.custom_cfg(19, 13, 136, nq=6, dtype=dtype, cid=320)
+    P, L = gc.make_pair(cfg)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    d = [gc.to_dev(a, L) for a in H]
+    res = {}
+    for n in (1, 3, 16):
+        L.set_work_scale(n)
+        two, fused = gc.fresh_out(L, len(names)), gc.fresh_out(L, len(names))
+        L.momentum(d[0], d[1], d[2], two[0], two[1], two[2])
+        L.scalars(d[3:], two[3:])
+        L.tendencies(d[0], d[1], d[2], fused[0], fused[1], fused[2], d[3:], fused[3:])
+        torch.cuda.synchronize()
+        assert "tma_fused" in L.describe_plan()
+        res[n] = (two, fused)
+    want = list(P.momentum(H[0], H[1], H[2])) + [P.scalar(H[0], H[1], H[2], q) for q in H[3:]]
+    for o, w_, nm in zip(res[16][1], want, names):
+        gc.check(cfg, o, w_, nm)
+        gc.check_halo_untouched(cfg, o, nm)
+    for n in (3, 16):
+        for a, b in zip(res[1][0] + res[1][1], res[n][0] + res[n][1]):
+            assert torch.equal(a, b), f"work scale {n} changed a result"
+    # the knob is for the flux form, overwrite mode, TMA kernels only
+    for bad in (lambda: L.set_form("pw_skew"), lambda: L.set_accumulate(True), lambda: L.set_variant("march"),
+                lambda: L.set_work_scale(0), lambda: L.set_work_scale(65)):
+        with pytest.raises(binding.MoncAdvError) as e:
+            bad()
+        assert e.value.code == binding.EINVAL
+    L.set_work_scale(1)
+    L.set_form("pw_skew")
+    with pytest.raises(binding.MoncAdvError):
+        L.set_work_scale(2)
+    L.close()
+    # a shape the TMA kernels do not take (odd nz): the compute call refuses while n > 1
+    cfg2 = gc.custom_cfg(5, 4, 9, dtype=dtype, cid=321)
+    P2, L2 = gc.make_pair(cfg2)
+    L2.set_work_scale(4)
+    z = [torch.zeros(L2.shape, device="cuda", dtype=L2.torch_dtype) for _ in range(6)]
+    with pytest.raises(binding.MoncAdvError) as e:
+        L2.momentum(*z)
+    assert e.value.code == binding.EINVAL
+    L2.close()
