@@ -204,8 +204,9 @@ TmaPlan compute_plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
   constexpr int NK = VecOf<T>::NK;
   if (h->nz % NK != 0) return pl;
   const int wzc = (h->nz / NK + 31) / 32;
-  if (wzc > kTmaMaxConsumerWarps) return pl;
-  const int tymax = std::min(h->ny, kTmaMaxConsumerWarps / wzc);
+  const int max_warps = tma_momentum_max_warps(h->accumulate != 0 || h->work > 1);
+  if (wzc > max_warps) return pl;
+  const int tymax = std::min(h->ny, max_warps / wzc);
   const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
   const int ty_hi = h->tile_y > 0 ? std::min(h->tile_y, tymax) : tymax;
   const int ty_lo = h->tile_y > 0 ? ty_hi : std::max(1, tymax - 3);
@@ -1112,6 +1113,7 @@ int monc_adv_set_form(monc_adv_t h, int form) {
 int monc_adv_set_accumulate(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
   if (on && h->work > 1) return fail(h, MONC_ADV_EINVAL, "set_accumulate: work scaling is on (overwrite mode only)");
+  if ((on ? 1 : 0) != h->accumulate) h->mom_plans.clear();  // the accumulating momentum kernel takes fewer warps
   h->accumulate = on ? 1 : 0;
   return MONC_ADV_OK;
 }
@@ -1121,6 +1123,7 @@ int monc_adv_set_work_scale(monc_adv_t h, int n) {
   if (n < 1 || n > 64) return fail(h, MONC_ADV_EINVAL, "set_work_scale: need 1 <= n <= 64");
   if (n > 1 && (h->form != MONC_ADV_FORM_FLUX || h->accumulate || (h->variant != 0 && h->variant != 3)))
     return fail(h, MONC_ADV_EINVAL, "set_work_scale: needs the flux form, overwrite mode and the TMA kernels");
+  if ((n > 1) != (h->work > 1)) h->mom_plans.clear();  // the work-scaled momentum kernel takes fewer warps
   h->work = n;
   return MONC_ADV_OK;
 }

@@ -25,6 +25,12 @@ namespace monc {
 
 constexpr int kTmaMaxConsumerWarps = 16;
 constexpr int kTmaThreads = kTmaMaxConsumerWarps * 32;
+// accumulate mode holds the three old tendencies of a point as well (and the work-scaled
+// variant every input of a step across its repetitions): with 128 registers
+// per thread (16 warps) the march spills inside its loop and the local-memory loads sit
+// on every step's critical path (2.3 x slower, measured); 14 warps leave 144 registers
+constexpr int kTmaMaxConsumerWarpsAcc = 14;
+constexpr int tma_momentum_max_warps(bool acc) { return acc ? kTmaMaxConsumerWarpsAcc : kTmaMaxConsumerWarps; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
   return (uint32_t)__cvta_generic_to_shared(p);
@@ -225,6 +231,14 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
   // The first step (plane i0-1 as the centre) only builds the x-face terms: no store.
   bool first = true;
   auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
+    // accumulate: what the tendencies are added to is read from global memory; issue those
+    // loads first so that their latency overlaps the wait for the plane and the arithmetic
+    Vec<T> au, av, aw;
+    if (ACC) {
+#pragma unroll
+      for (int e = 0; e < NK; ++e) au.v[e] = av.v[e] = aw.v[e] = T(0);
+      if (!first && m.act) { au = ld_vec_rw(m.su + c); av = ld_vec_rw(m.sv + c); aw = ld_vec_rw(m.sw + c); }
+    }
     mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
     chk_jitter(1);
     const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
@@ -278,7 +292,6 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
       if (m.act) {
         T *qu = m.su + c, *qv = m.sv + c, *qw = m.sw + c;
         if (ACC) {
-          const Vec<T> au = ld_vec_rw(qu), av = ld_vec_rw(qv), aw = ld_vec_rw(qw);
 #pragma unroll
           for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
         }
@@ -318,7 +331,7 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
 // mbarriers.
 // ---------------------------------------------------------------------------
 template <typename T, bool ACC, bool SKEW, bool WS = false>
-__global__ void __launch_bounds__(kTmaThreads, 1)
+__global__ void __launch_bounds__(tma_momentum_max_warps(ACC || WS) * 32, 1)
 tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__restrict__ u,
              const T *__restrict__ v, const T *__restrict__ w, T *__restrict__ su,
              T *__restrict__ sv, T *__restrict__ sw) {
@@ -590,15 +603,17 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
           evaluate(q);
         }
         CA[s] = can;
-        if (STORE && act) {  // sq of the previous plane is complete
+        if (STORE) {  // sq of the previous plane is complete
           o.v[0] = keep_if(o.v[0], keep_first);
           T *sq = sqp[s] + c;  // pointer table lives in the constant bank
           if (ACC) {
-            const Vec<T> a = ld_vec_rw(sq);
+            if (act) {
+              const Vec<T> a = ld_vec_rw(sq);
 #pragma unroll
-            for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
+              for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
+            }
           }
-          st_vec(sq, o);
+          if (act) st_vec(sq, o);  // nothing but the store under the predicate
         }
         pQ += fb;
       }
@@ -636,7 +651,8 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   constexpr int RS = kRowBytes / SZ;         // row stride in elements
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(kFull, (int)(threadIdx.x >> 5), 0);  // tells the compiler it is warp-uniform
   const int rows = ty + 2;
   const int stagesz = (3 + gb) * fieldsz;
   const uint32_t t0 = smem_u32(smem_raw);
@@ -710,7 +726,8 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   // u(column, k0) in stage 0: row col+1 of the box, one vector of z halo before level kb0
   const uint32_t a0 = t0 + (uint32_t)(((col + 1) * RS + (k0 - kb0 + NK)) * SZ);
   const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
-  const int keep_first = k0 == 0 ? 0 : -1;  // element 0 is level K = 1: no tendency
+  int keep_first = k0 == 0 ? 0 : -1;  // element 0 is level K = 1: no tendency
+  asm volatile("" : "+r"(keep_first));  // keep it a mask for a logic op: no compare + select per store
   if (MOM && sp == ss) {
     // ---------------- momentum role (fused launch): su, sv, sw of this column chunk
     // from the wind tiles the scalar warps use
