@@ -265,7 +265,11 @@ class Ctx:
         torch.cuda.set_device(self.local)
         if self.world > 1:
             import torch.distributed as dist
-            # NCCL_DEBUG=INFO (set by the caller) shows the communicator over all N ranks
+            # the communicator's own log (one "comm ... nranks N" line per rank) goes to stderr,
+            # so that a reader of the run can see that N ranks took part; stdout stays one JSON line
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
             dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
             self.dist = dist
 
