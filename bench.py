@@ -175,11 +175,9 @@ def config_record(cfg, workload, **extra):
 # kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
 # by (workload, kernel family); valid for the library's default launch plan only.
 NCU_TRAFFIC = {
-    ("config1", "tma_momentum"): (358.1e6, "profiles/r01_config1_tma_momentum_f64.md"),
-    ("config2", "tma_scalars"): (12814.3e6, "profiles/r01_config2_tma_scalars_f64.md"),
-    ("config3", "tma_scalars"): (6206.1e6, "profiles/r01_config3_tma_f32.md"),
-    ("config2", "tma_fused"): (14273.8e6, "profiles/r01_config2_tma_fused.md"),
-    ("config3", "tma_fused"): (7077.1e6, "profiles/r01_config3_tma_fused.md"),
+    ("config1", "tma_momentum"): (357.2e6, "profiles/r02_config1_tma_momentum.md"),
+    ("config2", "tma_fused"): (14918.3e6, "profiles/r02_config2_tma_fused.md"),
+    ("config3", "tma_fused"): (7126.1e6, "profiles/r02_config3_tma_fused.md"),
 }
 
 
@@ -445,7 +443,7 @@ def run_device_config(ctx, args, workload, cache, headline):
                         "algorithmic_GBs": bg, "frac": bg / roof["peak"], "frac_of_nominal_8TBs": bg / NOMINAL_GBS}
     # ---- the paper's work-scaling experiment: the flux arithmetic of every
     # point evaluated 16 times on the same bytes (ULTIMATE's cost); same results
-    if headline and not swap and not is_tuned(args):
+    if headline and not swap and not is_tuned(args) and not args.no_work_scale:
         ctx.barrier()
         time.sleep(1.0)
         L.set_work_scale(16)
@@ -794,6 +792,8 @@ def main():
     ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--no-others", action="store_true",
                     help="skip the compact records of the other BASELINE configs")
+    ap.add_argument("--no-work-scale", action="store_true",
+                    help="skip the x16 work-scaled leg (PAPER.md:109) of the headline record")
     ap.add_argument("--sustain-seconds", type=float, default=2.5,
                     help="length of the sustained loop of the headline step (0 = skip)")
     ap.add_argument("--xchunk", type=int, default=0)
