@@ -63,6 +63,7 @@ struct monc_adv_s {
   std::vector<double> tz_host[4];                        // as stored on the device
   const void *wind[3] = {nullptr, nullptr, nullptr};
   int form = MONC_ADV_FORM_FLUX, accumulate = 0, variant = 0, pdl = 1, fuse = 1, work = 1;
+  volatile double zero = 0.0;  // handed to the work-scaled kernels as a run-time 0
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
@@ -151,6 +152,7 @@ KParams<T> make_params(monc_adv_t h, int ia, int ib) {
   p.skew = h->form == MONC_ADV_FORM_PW_SKEW;
   p.prefetch = h->prefetch < 0 ? 0 : (h->prefetch == 0 ? kDefaultPrefetch : h->prefetch);
   p.work = h->work;
+  p.zero = (T)h->zero;
   p.cx = (T)(1.0 / (4.0 * h->dx));
   p.cy = (T)(1.0 / (4.0 * h->dy));
   p.tzc1 = (const T *)h->d_tz[0]; p.tzc2 = (const T *)h->d_tz[1];
@@ -405,7 +407,9 @@ TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mo
           const int tiles = ((h->ny + ty - 1) / ty) * nzt * ngroups;
           // the groups after the first re-read the wind; about half of that hits L2
           const double wind = 3.0 * (1.0 + 0.5 * (ngroups - 1)) / ngroups;
-          const double dram_b = ((wind + gb) + gb + (mom ? 3 : 0)) * ty * ZB * sizeof(T);
+          // inputs: the two halo rows of a tile are re-reads; about 30 % of them miss L2
+          // (neighbouring blocks drift apart), fewer per byte in a taller tile
+          const double dram_b = ((wind + gb) * (1.0 + 0.6 / ty) + gb + (mom ? 3 : 0)) * ty * ZB * sizeof(T);
           const double t_mem = dram_b / (sm_gbs * 1e3);                            // us
           const double t_warp = std::max(0.15 + 0.25 * gw, mom ? 1.2 : 0.0);         // us; momentum ~ 4 scalars
           const double shallow = S >= 3 ? 1.0 : 1.15;

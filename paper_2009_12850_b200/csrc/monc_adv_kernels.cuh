@@ -46,6 +46,7 @@ struct KParams {
   int skew;         // generic kernels only: PW skew form
   int prefetch;     // march kernels: L2 prefetch distance in planes (0 = off)
   int work;         // TMA kernels, WS instantiations: evaluations of the flux arithmetic per point
+  T zero;           // 0, as a run-time value: x + zero * r is x, but no compiler can know it
   T cx, cy;         // 1/(4dx), 1/(4dy)
   const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz; tzc2[nz-1] = 0
 };
@@ -111,24 +112,31 @@ __device__ __forceinline__ Vec<T> ld_or_zero(const T *p, bool act) {
 
 constexpr unsigned kFull = 0xffffffffu;
 
-// the compiler must assume x changed: re-evaluations of the same arithmetic (the
-// work-scaling experiment of PAPER.md:109) are neither merged nor hoisted
-__device__ __forceinline__ void opaque(double &x) { asm volatile("" : "+d"(x)); }
-__device__ __forceinline__ void opaque(float &x) { asm volatile("" : "+f"(x)); }
+// Work scaling: repetition r of a point's arithmetic reads x + zero * r
+// (zero is a kernel parameter equal to 0: the value is x, but neither nvcc nor ptxas
+// can hoist the arithmetic out of the repetition loop), and `consume` makes every
+// repetition's results needed where they are produced, so they cannot be sunk out of
+// it either.
 template <typename T>
-__device__ __forceinline__ void opaque(Vec<T> &a) {
+__device__ __forceinline__ Vec<T> same_value(const Vec<T> &a, const T zero, const int r) {
+  Vec<T> o;
 #pragma unroll
-  for (int e = 0; e < VecOf<T>::NK; ++e) opaque(a.v[e]);
+  for (int e = 0; e < VecOf<T>::NK; ++e) o.v[e] = zero * (T)r + a.v[e];
+  return o;
+}
+__device__ __forceinline__ void consume(const double x) { asm volatile("" ::"d"(x)); }
+__device__ __forceinline__ void consume(const float x) { asm volatile("" ::"f"(x)); }
+template <typename T>
+__device__ __forceinline__ void consume(const Vec<T> &a) {
+#pragma unroll
+  for (int e = 0; e < VecOf<T>::NK; ++e) consume(a.v[e]);
 }
 
-__device__ __forceinline__ void prefetch_l2(const void *p) {
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
+
 // TMA-issued L2 prefetch of a contiguous run (bytes % 16 == 0, 16-B aligned)
 __device__ __forceinline__ void prefetch_l2_bulk(const void *p, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
-
 
 // value one level above each element: r[e] = a[e+1]; the last comes from the
 // next lane's first element, or (warp's last lane) from `edge`.

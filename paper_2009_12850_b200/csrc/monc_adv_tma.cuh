@@ -194,6 +194,7 @@ struct MarchArgs {
   uint32_t a0, fb, sbytes, rsb, bar0;
   int nstages, nsteps, lane;
   int work;  // WS: evaluations of the arithmetic per step (results identical)
+  T zero;    // WS: 0 as a run-time value (same_value)
   bool act, bot_edge;
   bool first_level, last_level;  // element 0 is level K = 1 (no tendency) / element NK-1 is level K = nz (sw = 0)
   T *su, *sv, *sw;            // output arrays (kernel parameters: re-read from the constant bank, not kept in registers)
@@ -272,10 +273,12 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
       // times on the same bytes; every evaluation gives the same result
 #pragma unroll 1
       for (int r = 0; r < m.work; ++r) {
-        PlaneRegs<T> &Rc = const_cast<PlaneRegs<T> &>(RC);  // the registers themselves, values unchanged
-        opaque(Rc.u); opaque(Rc.v); opaque(Rc.vs); opaque(Rc.w);
+        PlaneRegs<T> Rc;
+        Rc.u = same_value(RC.u, m.zero, r); Rc.v = same_value(RC.v, m.zero, r);
+        Rc.vs = same_value(RC.vs, m.zero, r); Rc.w = same_value(RC.w, m.zero, r);
         momentum_faces<T, SKEW>(Rc, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz,
                                 m.c1, m.c2, m.d1, m.d2, m.cx, m.cy, lane, ou, ov, ow);
+        consume(ou); consume(ov); consume(ow); consume(FE.xx); consume(FE.xy); consume(FE.xz);
       }
     } else {
       momentum_faces<T, SKEW>(RC, RE, FW, FE, uS, uN, vN, wS, wN, uCu, vCu, wCu, vSu, b_xz, b_yz, b_zz, m.c1,
@@ -402,7 +405,7 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   m.a0 = t0 + (uint32_t)(((col + 1) * nz + k0) * SZ);  // u(column, k0) in stage 0
   m.fb = fb; m.sbytes = sb; m.rsb = (uint32_t)(nz * SZ); m.bar0 = bar0;
   m.nstages = nstages; m.nsteps = nsteps; m.lane = lane;
-  m.work = p.work;
+  m.work = p.work; m.zero = p.zero;
   m.bot_edge = m.act && lane == 0 && zc > 0;
   m.first_level = k0 == 0;
   m.last_level = k0 + NK == nz;
@@ -504,7 +507,8 @@ constexpr int kRowBytes = 34 * 16;  // 32 vectors of the tile + one vector of z 
 template <typename T, int GW, bool ACC, bool SKEW, bool FULL, bool WS>
 __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t fb, const uint32_t sbytes,
                                              const uint32_t q0off, const uint32_t bar0, const int nstages,
-                                             const int nplanes, const int mycnt, const int work, const int lane,
+                                             const int nplanes, const int mycnt, const int work, const T zero,
+                                             const int lane,
                                              const bool act, const bool bot_edge, const int keep_first,
                                              T *const *__restrict__ sqp, const long long c0,
                                              const long long plane, const Vec<T> &c1, const Vec<T> &c2,
@@ -596,8 +600,8 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
           // the same arithmetic `work` times on the same bytes, same result
 #pragma unroll 1
           for (int r = 0; r < work; ++r) {
-            opaque(QN[s]);  // the registers themselves, values unchanged
-            evaluate(QN[s]);
+            evaluate(same_value(q, zero, r));
+            consume(o); consume(can);
           }
         } else {
           evaluate(q);
@@ -736,7 +740,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     m.d1 = ld_vec(p.tzd1 + k0); m.d2 = ld_vec(p.tzd2 + k0);
     m.a0 = a0; m.fb = fb; m.sbytes = sbytes; m.rsb = (uint32_t)kRowBytes; m.bar0 = bar0;
     m.nstages = nstages; m.nsteps = nplanes - 1; m.lane = lane;
-    m.work = p.work;
+    m.work = p.work; m.zero = p.zero;
     m.act = act; m.bot_edge = bot_edge;
     m.first_level = k0 == 0;
     m.last_level = k0 + NK == nz;
@@ -758,11 +762,11 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   T *const *sqp = outs.sq + (s0 + sb);
   pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
   if (mycnt == GW)
-    scalar_march<T, GW, ACC, SKEW, true, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, lane,
-                                             act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, true, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, p.zero,
+                                             lane, act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
   else
-    scalar_march<T, GW, ACC, SKEW, false, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, lane,
-                                              act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, false, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, p.zero,
+                                              lane, act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
 }
 
 }  // namespace monc

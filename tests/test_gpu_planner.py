@@ -91,6 +91,6 @@ def test_config2_and_3_fused_plan(cid):
 
 def test_config2_two_call_plans():
     knobs = [dict(), dict(xchunk=32), dict(xchunk=64), dict(xchunk=128), dict(xchunk=64, split=3),
-             dict(xchunk=64, group=5)]
+             dict(xchunk=64, group=5), dict(xchunk=64, tile_y=7), dict(xchunk=64, tile_y=5)]
     best, plans = _bench(synth.CONFIGS[2], knobs, _two_calls, steps=6)
     _check("config2 momentum + scalars", best, plans, knobs)
