@@ -177,8 +177,13 @@ int monc_adv_step_chunk_range(monc_adv_t h, int c, int *x_begin, int *x_end);
  * last D2H end, out[3] = whole step (first copy to last copy). */
 int monc_adv_step_times_ms(monc_adv_t h, float out[4]);
 
-/* Number of x-slab chunks of step_async (default 8, 1 <= n <= nx). */
+/* Number of x-slab chunks of step_async: 1 <= n <= nx, or 0 (the default) to let
+ * the library choose per step from the bytes on the host link and the fixed cost
+ * of a chunk (a step takes T (1 + 1/C) + C c). */
 int monc_adv_set_chunks(monc_adv_t h, int nchunks);
+/* Chunk count of the step in flight (or of the last one); with a fixed count, that
+ * count.  0 = automatic and no step enqueued yet. */
+int monc_adv_step_chunk_count(monc_adv_t h);
 /* 1 (default): copies and kernels overlap on separate streams.  0: the same
  * work serialised on one stream (H2D all, kernels, D2H all) -- the baseline
  * for the overlap ratio. */

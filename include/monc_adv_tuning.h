@@ -34,6 +34,12 @@ int monc_adv_set_variant(monc_adv_t h, int variant);
 int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
                         int tile_y, int split);
 
+/* Thread-block cluster size of the TMA kernels (1..8; 0 = library default): that
+ * many y-neighbour tiles are launched as one cluster, i.e. co-scheduled on the SMs
+ * of one GPC.  No shared-memory traffic crosses the cluster; it only keeps blocks
+ * that re-read each other's halo rows running at the same rate. */
+int monc_adv_set_cluster(monc_adv_t h, int n);
+
 /* 1 (default): the TMA kernels are launched with CUDA's programmatic
  * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
  * predecessor in the stream (it waits for the predecessor's completion before

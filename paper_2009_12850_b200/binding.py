@@ -28,11 +28,12 @@ MAX_SCALARS = 64
 SYMBOLS = [
     "monc_adv_create", "monc_adv_destroy", "monc_adv_momentum", "monc_adv_bind_wind",
     "monc_adv_scalars", "monc_adv_tendencies", "monc_adv_set_fuse", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
-    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range",
+    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range", "monc_adv_step_chunk_count",
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
     "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version", "monc_adv_set_work_scale",
+    "monc_adv_set_cluster",
 ]
 
 
@@ -89,11 +90,13 @@ def load():
     lib.monc_adv_step_wait_chunk.restype = ci
     lib.monc_adv_step_chunk_range.argtypes = [vp, ci, C.POINTER(ci), C.POINTER(ci)]
     lib.monc_adv_step_chunk_range.restype = ci
+    lib.monc_adv_step_chunk_count.argtypes = [vp]
+    lib.monc_adv_step_chunk_count.restype = ci
     lib.monc_adv_step_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
                  "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
-                 "monc_adv_set_fuse", "monc_adv_set_work_scale"):
+                 "monc_adv_set_fuse", "monc_adv_set_work_scale", "monc_adv_set_cluster"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -251,6 +254,9 @@ class MoncAdv:
         return dict(h2d=out[0], kernels=out[1], d2h=out[2], total=out[3])
 
     # -- settings ----------------------------------------------------------
+    def step_chunk_count(self) -> int:
+        return int(self._lib.monc_adv_step_chunk_count(self._h))
+
     def set_chunks(self, n):
         self._check(self._lib.monc_adv_set_chunks(self._h, int(n)))
 
@@ -266,6 +272,9 @@ class MoncAdv:
 
     def set_pdl(self, on):
         self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
+
+    def set_cluster(self, n):
+        self._check(self._lib.monc_adv_set_cluster(self._h, int(n)))
 
     def set_work_scale(self, n):
         self._check(self._lib.monc_adv_set_work_scale(self._h, int(n)))

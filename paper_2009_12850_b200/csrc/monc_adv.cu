@@ -29,10 +29,15 @@ namespace {
 thread_local std::string g_create_error;
 }
 
+// default thread-block cluster sizes (y-neighbour tiles co-scheduled on one GPC)
+constexpr int kDefaultClusterMomentum = 4;  // single-wave launches only
+constexpr int kDefaultClusterScalars = 1;
+
 // geometry of the TMA-staged kernels: TY columns per block, ring depth S
 struct TmaPlan {
   bool ok = false;
   int ty = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0;
+  int cl = 1;  // thread-block cluster: cl y-neighbour tiles are co-scheduled on one GPC
   size_t smem = 0;
 };
 // geometry of tma_scalars: ty columns x ss scalar splits = consumer warps per
@@ -41,6 +46,7 @@ struct TmaPlan {
 struct TmaScalarPlan {
   bool ok = false;
   int ty = 0, ss = 0, gb = 0, gw = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0, fieldsz = 0;
+  int cl = 1;  // thread-block cluster: cl y-neighbour tiles are co-scheduled on one GPC
   size_t smem = 0;
 };
 // tensor-map descriptors of one launch, kept while the same arrays come back
@@ -66,6 +72,7 @@ struct monc_adv_s {
   volatile double zero = 0.0;  // handed to the work-scaled kernels as a run-time 0
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
+  int cluster = 0;                                      // TMA kernels: y tiles per thread-block cluster, 0 = default
   int smem_optin = 0;                                   // max dynamic smem per block
   long launches = 0;
   std::string err;
@@ -76,7 +83,7 @@ struct monc_adv_s {
   std::vector<MapEntry> map_cache;
   unsigned long map_clock = 0;
   // ---- async step state
-  int nchunks = 8, overlap = 1;
+  int nchunks = 0, overlap = 1;  // nchunks 0 = chosen per step (auto_chunks)
   int staged_nq = -1;
   std::vector<void *> d_in, d_out;  // 3+nq each
   cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
@@ -239,6 +246,14 @@ TmaPlan compute_plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
       }
     }
   }
+  if (pl.ok) {
+    // a single wave is placed 4 y-neighbour blocks at a time: 16 (or 20) blocks per GPC instead
+    // of whatever the block scheduler deals out, +2 % at config 1; several
+    // waves gain nothing from it (and clusters of 8 leave most of a GPC idle)
+    const bool one_wave = (long)pl.tiles * pl.nchunks <= h->sm_count;
+    const int want = h->cluster > 0 ? h->cluster : (one_wave ? kDefaultClusterMomentum : 1);
+    pl.cl = std::max(1, std::min(want, pl.tiles));
+  }
   return pl;
 }
 
@@ -270,18 +285,26 @@ cudaError_t allow_max_smem(monc_adv_t h, K kernel) {
 // may begin (barrier set-up, coefficient loads) while its predecessor in the
 // stream drains; it calls griddepcontrol.wait before touching any field.
 template <typename... KArgs, typename... Args>
-cudaError_t launch_pdl(monc_adv_t h, void (*kernel)(KArgs...), dim3 grid, int threads, size_t smem,
+cudaError_t launch_pdl(monc_adv_t h, void (*kernel)(KArgs...), dim3 grid, int cluster, int threads, size_t smem,
                        cudaStream_t st, Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3((unsigned)threads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = h->pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  if (cluster > 1) {
+    // `cluster` consecutive blocks in x (y-neighbour tiles) run together on one GPC
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = (unsigned)cluster;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    cfg.numAttrs = 2;
+  }
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
@@ -297,10 +320,10 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
   if (h->work > 1 && !pl.ok) return fail(h, MONC_ADV_EINVAL, "momentum: work scaling needs the TMA kernels");
   if (pl.ok) {
     p.xc = pl.xc;
-    dim3 grid(pl.tiles, pl.nchunks);
+    dim3 grid((pl.tiles + pl.cl - 1) / pl.cl * pl.cl, pl.nchunks);  // padded to whole clusters: the extra blocks exit
     auto go = [&](auto kernel) -> int {
       CU(allow_max_smem(h, kernel));
-      CU(launch_pdl(h, kernel, grid, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages, u, v, w, su, sv, sw));
+      CU(launch_pdl(h, kernel, grid, pl.cl, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages, u, v, w, su, sv, sw));
       return MONC_ADV_OK;
     };
     const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
@@ -309,8 +332,8 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
                                    : (skew ? go(tma_momentum<T, false, true>) : go(tma_momentum<T, false, false>));
     if (rc != MONC_ADV_OK) return rc;
     char b[160];
-    snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d threads=%d smem=%zu", pl.ty,
-             pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.ty * p.wzc * 32, pl.smem);
+    snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d cluster=%d threads=%d smem=%zu", pl.ty,
+             pl.stages, pl.xc, (int)grid.x, pl.nchunks, pl.cl, pl.ty * p.wzc * 32, pl.smem);
     h->plan_mom = b;
   } else if (use_march<T>(h)) {
     const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
@@ -439,6 +462,14 @@ TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mo
       }
     }
   }
+  if (pl.ok && (n + pl.gb - 1) / pl.gb == 1) {
+    // one scalar group: cl y-neighbour tiles (same z tile) form a thread-block cluster; the
+    // tile count is padded to whole clusters (the extra blocks exit at once)
+    constexpr int ZB = 32 * NK;
+    const int nzt = (h->nz + ZB - 1) / ZB, nyt = (h->ny + pl.ty - 1) / pl.ty;
+    pl.cl = std::max(1, std::min(h->cluster > 0 ? h->cluster : kDefaultClusterScalars, nyt));
+    pl.tiles = (nyt + pl.cl - 1) / pl.cl * pl.cl * nzt;
+  }
   return pl;
 }
 
@@ -498,8 +529,8 @@ int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &ma
   CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>));
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>, grid, threads, pl.smem, st, p, maps, outs, mo, nq,
-                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz));
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>, grid, pl.cl, threads, pl.smem, st, p, maps, outs, mo, nq,
+                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz, pl.cl));
   return MONC_ADV_OK;
 }
 
@@ -558,9 +589,9 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
     CU(cudaGetLastError());
     h->launches++;
     char b[200];
-    snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d stages=%d xc=%d grid=%dx%d "
+    snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d stages=%d xc=%d grid=%dx%d cluster=%d "
              "threads=%d smem=%zu", mo ? "tma_fused(momentum+scalars)" : "tma_scalars", pl.gb, pl.gw, pl.ss,
-             pl.ty, pl.stages, pl.xc, pl.tiles, pl.nchunks, (pl.ty * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
+             pl.ty, pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.cl, (pl.ty * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
     h->plan_sca = b;
     if (mo) h->plan_mom.clear();
   }
@@ -652,7 +683,29 @@ void free_staging(monc_adv_t h) {
   h->staged_nq = -1;
 }
 
-int ensure_async_objects(monc_adv_t h, int nq) {
+// Chunk count of a hybrid step when the caller did not fix one.  Both copy engines run
+// flat out, D2H one chunk behind H2D, so a step takes T (1 + 1/C) + C c: T = the time of
+// one direction's bytes on the host link, c = the fixed cost of a chunk (its copies' set-up,
+// events, a kernel launch).  Minimum at C = sqrt(T / c).  Measured on B200 / PCIe Gen5 x16
+// (DESIGN.md 7.3): both directions at once move 49.5 GB/s each, c = 15 us + 5 us per copy
+// (config 4: 212 ms at C = 8, 201 ms at 32..64; config 2: 158 ms at 8, 151 ms at 32; config 1's shape: 8).
+int auto_chunks(monc_adv_t h, int nf_in, int nf_out) {
+  const double bytes = (double)std::max(nf_in, nf_out) * (double)h->nx * h->nyh * h->nz * (double)h->esize;
+  const double t_ms = bytes / 49.5e6;
+  const double c_ms = 0.015 + 0.005 * (nf_in + nf_out);
+  // the power of two nearest to sqrt(T / c): equal slabs copy measurably better than ragged
+  // ones (config 2: 150.9 ms at C = 32, 156 ms at 31 and 33), and the minimum is flat
+  const double want = std::sqrt(t_ms / c_ms);
+  int c = 1;
+  while (c < 64 && (double)(2 * c) * (2 * c) <= want * want * 2.0) c *= 2;  // 2c <= want * sqrt(2)
+  while (c > h->nx) c /= 2;
+  return std::max(1, c);
+}
+int step_chunks(monc_adv_t h, int nf_in, int nf_out) {
+  return h->nchunks > 0 ? std::min(h->nchunks, h->nx) : auto_chunks(h, nf_in, nf_out);
+}
+
+int ensure_async_objects(monc_adv_t h, int nq, int nchunks) {
   if (!h->s_in) {
     CU(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
     CU(cudaStreamCreateWithFlags(&h->s_k, cudaStreamNonBlocking));
@@ -661,7 +714,7 @@ int ensure_async_objects(monc_adv_t h, int nq) {
     CU(cudaEventCreate(&h->ev_in_begin));
     CU(cudaEventCreate(&h->ev_out_begin));
   }
-  while ((int)h->ev_h2d.size() < h->nchunks) {
+  while ((int)h->ev_h2d.size() < nchunks) {
     cudaEvent_t a, b, c, d;
     CU(cudaEventCreate(&a)); CU(cudaEventCreate(&b));
     CU(cudaEventCreate(&c)); CU(cudaEventCreate(&d));
@@ -710,7 +763,7 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
                     const void *const *hq, int nq, void *hsu, void *hsv, void *hsw,
                     void *const *hsq, cudaStream_t user) {
   const bool mom = hsu != nullptr;
-  const int C = std::min(h->nchunks, h->nx);
+  const int C = step_chunks(h, 3 + nq, ((mom ? 3 : 0) + nq) * (h->accumulate ? 2 : 1));
   const size_t es = sizeof(T);
   const size_t plane_b = (size_t)h->nyh * h->nz * es;
   const int nf = 3 + nq;
@@ -1017,7 +1070,7 @@ int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void
       if (!is_pinned_host(p, bytes))
         return fail(h, MONC_ADV_EINVAL, "step_async: every host array must be page-locked (pinned) over its "
                                         "whole length; pageable memory would make the copies synchronous");
-  rc = ensure_async_objects(h, nq);
+  rc = ensure_async_objects(h, nq, step_chunks(h, 3 + nq, ((hsu ? 3 : 0) + nq) * (h->accumulate ? 2 : 1)));
   if (rc) return rc;
   cudaStream_t user = (cudaStream_t)cuda_stream;
   rc = h->dtype == MONC_ADV_F64 ? step_async_impl<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user)
@@ -1074,9 +1127,16 @@ int monc_adv_step_wait(monc_adv_t h) {
   return MONC_ADV_OK;
 }
 
+int monc_adv_step_chunk_count(monc_adv_t h) {
+  if (!h) return 0;
+  if (h->nchunks > 0) return std::min(h->nchunks, h->nx);
+  return (int)h->chunk_a.size();  // automatic: known once a step has been enqueued
+}
+
 int monc_adv_step_chunk_range(monc_adv_t h, int c, int *x_begin, int *x_end) {
   if (!h) return MONC_ADV_EINVAL;
-  const int C = std::min(h->nchunks, h->nx);
+  const int C = monc_adv_step_chunk_count(h);
+  if (C == 0) return fail(h, MONC_ADV_EINVAL, "step_chunk_range: automatic chunk count and no step enqueued yet");
   if (c < 0 || c >= C || !x_begin || !x_end) return fail(h, MONC_ADV_EINVAL, "step_chunk_range: bad argument");
   *x_begin = (int)((long long)h->nx * c / C);
   *x_end = (int)((long long)h->nx * (c + 1) / C);
@@ -1093,8 +1153,10 @@ int monc_adv_step_times_ms(monc_adv_t h, float out[4]) {
 int monc_adv_set_chunks(monc_adv_t h, int nchunks) {
   if (!h) return MONC_ADV_EINVAL;
   if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_chunks: step in flight");
-  if (nchunks < 1 || nchunks > h->nx) return fail(h, MONC_ADV_EINVAL, "set_chunks: need 1 <= nchunks <= nx");
+  if (nchunks < 0 || nchunks > h->nx) return fail(h, MONC_ADV_EINVAL, "set_chunks: need 0 (automatic) or 1 <= nchunks <= nx");
   h->nchunks = nchunks;
+  h->chunk_a.clear();
+  h->chunk_b.clear();
   return MONC_ADV_OK;
 }
 
@@ -1129,6 +1191,15 @@ int monc_adv_set_work_scale(monc_adv_t h, int n) {
     return fail(h, MONC_ADV_EINVAL, "set_work_scale: needs the flux form, overwrite mode and the TMA kernels");
   if ((n > 1) != (h->work > 1)) h->mom_plans.clear();  // the work-scaled momentum kernel takes fewer warps
   h->work = n;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_cluster(monc_adv_t h, int n) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (n < 0 || n > 8) return fail(h, MONC_ADV_EINVAL, "set_cluster: 0 (default) or 1..8");
+  h->cluster = n;
+  h->mom_plans.clear();
+  h->sca_plans.clear();
   return MONC_ADV_OK;
 }
 

@@ -349,6 +349,7 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   const uint32_t bar0 = smem_u32(smem_raw + (size_t)nstages * stagesz * sizeof(T));
   // full[s] at bar0 + 8 s, empty[s] at bar0 + 8 (nstages + s)
   const int jr0 = blockIdx.x * ty;
+  if (jr0 >= p.ny) return;  // grid padded to whole thread-block clusters
   const int ncol = min(ty, p.ny - jr0);
   const int i0 = p.ia + blockIdx.y * p.xc;
   const int i1 = min(p.ib, i0 + p.xc);
@@ -648,7 +649,7 @@ template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const MomPtrs<T> mo, const int nq, const int ngroups, const int gb, const int ty,
-            const int ss, const int nstages, const int fieldsz) {
+            const int ss, const int nstages, const int fieldsz, const int cl) {
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
   constexpr int ZB = 32 * NK;                // levels per block tile
@@ -668,7 +669,13 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   const int grp = blockIdx.x % ngroups;
   const int tile = blockIdx.x / ngroups;
   const int nzt = (nz + ZB - 1) / ZB;
-  const int zt = tile % nzt, yt = tile / nzt;
+  // `cl` consecutive blocks are one thread-block cluster: y-neighbour tiles of the same z
+  // tile, co-scheduled on one GPC so that they advance at the same rate and find each
+  // other's halo rows in L2 (cl = 1: z tile fastest).  Tiles past the last y tile pad the
+  // grid to whole clusters and exit.
+  const int cidx = tile / cl, crank = tile - cidx * cl;
+  const int zt = cidx % nzt, yt = (cidx / nzt) * cl + crank;
+  if (yt * ty >= p.ny) return;
   const int s0 = grp * gb;
   const int cnt = min(gb, nq - s0);  // scalars of this block
   const int jr0 = yt * ty;

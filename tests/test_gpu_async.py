@@ -82,6 +82,47 @@ def test_step_async_small(nchunks, overlap, dtype):
     L.close()
 
 
+def test_step_async_automatic_chunk_count():
+    # monc_adv_set_chunks(h, 0), the default: the library picks the count per step from the bytes
+    # on the host link (T (1 + 1/C) + C c); the count is known once a step is enqueued
+    cfg = gc.custom_cfg(40, 24, 64, nq=2, cid=405)
+    P, L = gc.make_pair(cfg)
+    assert L.step_chunk_count() == 0  # automatic, nothing enqueued yet
+    with pytest.raises(binding.MoncAdvError) as e:
+        L.step_chunk_range(0)
+    assert e.value.code == binding.EINVAL
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    names = synth.field_names(cfg)
+    Q = [synth.field(cfg, n) for n in names]
+    hin = [pinned(a, L) for a in (U, V, W)]
+    hq = [pinned(a, L) for a in Q]
+    hout, hsq = pinned_out(L, 3), pinned_out(L, 2)
+    L.step_async(*hin, hq, *hout, hsq)
+    C = L.step_chunk_count()
+    assert 1 <= C <= cfg.nx
+    covered = []
+    for c in range(C):
+        L.step_wait_chunk(c)
+        covered.append(L.step_chunk_range(c))
+    assert covered[0][0] == 0 and covered[-1][1] == cfg.nx
+    assert all(a[1] == b[0] for a, b in zip(covered[:-1], covered[1:]))
+    L.step_wait()
+    for o, w_, n in zip(hout, P.momentum(U, V, W), ("su", "sv", "sw")):
+        gc.check(cfg, o, w_, n)
+        gc.check_halo_untouched(cfg, o, n)
+    for o, q, n in zip(hsq, Q, names):
+        gc.check(cfg, o, P.scalar(U, V, W, q), n)
+    # a fixed count again: known without a step, and the result does not depend on it
+    L.set_chunks(3)
+    assert L.step_chunk_count() == 3
+    hout2, hsq2 = pinned_out(L, 3), pinned_out(L, 2)
+    L.step_async(*hin, hq, *hout2, hsq2)
+    L.step_wait()
+    for a_, b_ in zip(hout + hsq, hout2 + hsq2):
+        assert torch.equal(a_, b_)
+    L.close()
+
+
 def test_step_async_pw_skew():
     # the hybrid step in the PW-skew form (NEXT-1): x-slab launches of the TMA kernels
     cfg = gc.custom_cfg(24, 17, 128, nq=4, cid=403)
