@@ -30,6 +30,14 @@
  *   - No output array may overlap an input array or another output array
  *     (checked over the whole arrays, not only the base pointers: EINVAL).  All
  *     base pointers must be 16-byte aligned.
+ *   - Shapes: any nx, ny >= 1, nz >= 3, halo >= 1.  The fast (TMA) kernels take
+ *     every nz for which nz * sizeof(dtype) is a multiple of 16 bytes, and a
+ *     "ragged" nz (any other) when ny + 2 halo is a multiple of 2 (fp64; fp32
+ *     with even nz) or of 4 (fp32 with odd nz), at about 0.9 of the aligned rate
+ *     in fp64; the remaining shapes run one-thread-per-point
+ *     kernels (about 0.4).  With a ragged nz the value above a column's top level
+ *     is read from the neighbouring column and multiplied by a zero coefficient:
+ *     inputs must be finite.
  *   - Every call returns MONC_ADV_OK (0) or a negative error code, never
  *     throws or aborts; monc_adv_last_error gives the text of the last
  *     failure on that handle.

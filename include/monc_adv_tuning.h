@@ -16,8 +16,9 @@ extern "C" {
 
 /* Kernel variant: 0 = auto (default), 1 = generic one-thread-per-point
  * kernels, 2 = x-marching vector kernels with direct global loads, 3 =
- * x-marching kernels fed by a TMA shared-memory ring.  2 and 3 need
- * nz % (16/sizeof(dtype)) == 0; 2 also needs the flux form. */
+ * x-marching kernels fed by a TMA shared-memory ring.  2 needs
+ * nz % (16/sizeof(dtype)) == 0 and the flux form; 3 takes a ragged nz too when
+ * ny + 2 halo is a multiple of 2 (fp64, fp32 with even nz) or 4 (fp32, odd nz). */
 int monc_adv_set_variant(monc_adv_t h, int variant);
 /* Tuning knobs of the x-marching kernels; 0 = library default, -1 = off where
  * that makes sense.

@@ -23,7 +23,7 @@ DEPS = SOURCES + [os.path.join(CSRC, "monc_adv_kernels.cuh"),
                   os.path.join(ROOT, "include", "monc_adv.h"),
                   os.path.join(ROOT, "include", "monc_adv_tuning.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-split-compile", "0",
          "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
          "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

@@ -61,6 +61,10 @@ struct MapEntry {
 struct monc_adv_s {
   int nx = 0, ny = 0, nz = 0, h = 0, dtype = 0;
   int nxh = 0, nyh = 0;
+  // tensor-map view of a field for tma_scalars: `colgroup` columns form one row, so that a row
+  // is a whole number of 16-byte vectors whatever nz is (1 when nz already is; 2 or 4 when nz is
+  // ragged; 0 = no such view: nyh is not a multiple of it, the generic kernels run)
+  int colgroup = 1;
   double dx = 0, dy = 0;
   size_t elems = 0, esize = 8;
   int device = 0;
@@ -152,6 +156,7 @@ KParams<T> make_params(monc_adv_t h, int ia, int ib) {
   p.plane = (long long)h->nyh * h->nz;
   p.ia = ia; p.ib = ib;
   constexpr int NK = VecOf<T>::NK;
+  p.colgroup = std::max(1, h->colgroup);
   p.wzc = (h->nz / NK + 31) / 32;
   p.units = h->ny * p.wzc;
   p.xc = ib - ia;
@@ -309,13 +314,19 @@ cudaError_t launch_pdl(monc_adv_t h, void (*kernel)(KArgs...), dim3 grid, int cl
 }
 
 template <typename T>
+int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T *w, const void *const *q,
+                    void *const *sq, int nq, int ia, int ib, cudaStream_t st, bool *done,
+                    const MomPtrs<T> *mo = nullptr);
+
+template <typename T>
 int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
                     int ia, int ib, cudaStream_t st) {
   if (ib <= ia) return MONC_ADV_OK;
   KParams<T> p = make_params<T>(h, ia, ib);
   TmaPlan pl;
   if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia);
-  if (h->variant == 3 && !pl.ok)
+  const bool ragged = h->nz % VecOf<T>::NK != 0 && h->colgroup > 1;  // served by the tensor-map kernel's momentum role
+  if (h->variant == 3 && !pl.ok && !ragged)
     return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
   if (h->work > 1 && !pl.ok) return fail(h, MONC_ADV_EINVAL, "momentum: work scaling needs the TMA kernels");
   if (pl.ok) {
@@ -335,6 +346,18 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
     snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d cluster=%d threads=%d smem=%zu", pl.ty,
              pl.stages, pl.xc, (int)grid.x, pl.nchunks, pl.cl, pl.ty * p.wzc * 32, pl.smem);
     h->plan_mom = b;
+  } else if (ragged && (h->variant == 0 || h->variant == 3)) {
+    // ragged nz: tma_momentum's 1-D bulk copies need whole vectors per column; the momentum
+    // role of the tensor-map kernel does not
+    bool done = false;
+    const MomPtrs<T> mo{su, sv, sw};
+    const int rc = run_tma_scalars<T>(h, p, u, v, w, nullptr, nullptr, 0, ia, ib, st, &done, &mo);
+    if (rc != MONC_ADV_OK) return rc;
+    if (done) return MONC_ADV_OK;
+    if (h->variant == 3) return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this shape");
+    h->plan_mom = "generic_momentum";
+    const long long n = (long long)(ib - ia) * h->ny * h->nz;
+    generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
   } else if (use_march<T>(h)) {
     const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
     const int bx = (p.units + wpb - 1) / wpb;
@@ -376,13 +399,16 @@ EncodeTiledFn tensor_map_encoder() {
 }
 
 // descriptor of one field F[NXH][NYH][nz] with a (z, y, x) box of box_z x box_y x 1
+// (colgroup G > 1, ragged nz: G columns per row of the view, a box holds the rows of one class of
+// columns j mod G of the tile; tma_scalars' producer)
 template <typename T>
 bool encode_field_map(monc_adv_t h, CUtensorMap *m, const void *base, int box_z, int box_y) {
   EncodeTiledFn enc = tensor_map_encoder();
   if (!enc) return false;
-  const cuuint64_t gdim[3] = {(cuuint64_t)h->nz, (cuuint64_t)h->nyh, (cuuint64_t)h->nxh};
-  const cuuint64_t gstr[2] = {(cuuint64_t)h->nz * sizeof(T), (cuuint64_t)h->nyh * h->nz * sizeof(T)};
-  const cuuint32_t box[3] = {(cuuint32_t)box_z, (cuuint32_t)box_y, 1u};
+  const int G = std::max(1, h->colgroup);
+  const cuuint64_t gdim[3] = {(cuuint64_t)G * h->nz, (cuuint64_t)(h->nyh / G), (cuuint64_t)h->nxh};
+  const cuuint64_t gstr[2] = {(cuuint64_t)G * h->nz * sizeof(T), (cuuint64_t)h->nyh * h->nz * sizeof(T)};
+  const cuuint32_t box[3] = {(cuuint32_t)box_z, (cuuint32_t)(G > 1 ? ragged_class_rows(box_y, G) : box_y), 1u};
   const cuuint32_t estr[3] = {1u, 1u, 1u};
   const CUtensorMapDataType dt =
       sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
@@ -395,7 +421,8 @@ template <typename T>
 TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom) {
   TmaScalarPlan pl;
   constexpr int NK = VecOf<T>::NK;
-  if (h->nz % NK != 0 || !tensor_map_encoder()) return pl;
+  if (h->colgroup == 0 || !tensor_map_encoder()) return pl;
+  if (n == 0 && !mom) return pl;
   const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
   const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
   double best = 1e300;
@@ -405,24 +432,26 @@ TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mo
   // the ring has only two stages, plus a fixed synchronisation cost; a launch takes
   // waves * (planes per block + 4) steps.
   const double sm_gbs = 6200.0 / h->sm_count;
-  for (int gb = std::min(n, 10); gb >= 1; --gb) {
+  // n = 0 (momentum only through the momentum role: ragged nz, where tma_momentum's 1-D bulk
+  // copies cannot be used): no scalar warps, gb = ss = 0
+  for (int gb = std::min(n, 10); gb >= (n == 0 ? 0 : 1); --gb) {
     if (h->group > 0 && gb != std::min(h->group, std::min(n, 10))) continue;
     if (h->group == 0 && gb != std::min(n, 5) && gb != std::min(n, 10)) continue;
-    const int ngroups = (n + gb - 1) / gb;
+    const int ngroups = gb == 0 ? 1 : (n + gb - 1) / gb;
     if (mom && ngroups != 1) continue;  // the momentum role runs once: one group holds every scalar
-    for (int ss = 1; ss <= std::min(gb, 4); ++ss) {
-      if (h->split > 0 && ss != std::min(h->split, std::min(gb, 4))) continue;
-      const int gw = (gb + ss - 1) / ss;
+    for (int ss = (gb == 0 ? 0 : 1); ss <= std::min(gb, 4); ++ss) {
+      if (gb > 0 && h->split > 0 && ss != std::min(h->split, std::min(gb, 4))) continue;
+      const int gw = gb == 0 ? 1 : (gb + ss - 1) / ss;
       if (gw > 5) continue;
       {
         // one 32-vector z chunk per block tile: the row stride is a compile-time constant
-        const int ZB = 32 * NK, RS = kRowBytes / (int)sizeof(T);
-        const int nzt = (h->nz + ZB - 1) / ZB;
+        const int ZB = 32 * NK;
+        const int nzt = scalar_z_tiles(h->nz, NK, h->colgroup, h->nz % NK != 0);
         const int tymax = std::min(h->ny, kScalarConsumerWarps / (ss + (mom ? 1 : 0)));
         if (tymax < 1) continue;
         for (int ty = tymax; ty >= 1; --ty) {
           if (h->tile_y > 0 && ty != std::min(h->tile_y, tymax)) continue;
-          const size_t field = ((size_t)(ty + 2) * RS * sizeof(T) + 127) / 128 * 128;
+          const size_t field = (size_t)scalar_field_bytes(ty + 2, h->colgroup, h->nz % NK != 0);
           const size_t stage = (size_t)(3 + gb) * field;
           int S = (int)std::min<size_t>(8, budget / (stage + 16));
           if (h->stages > 0) S = std::min(S, h->stages);
@@ -462,11 +491,10 @@ TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mo
       }
     }
   }
-  if (pl.ok && (n + pl.gb - 1) / pl.gb == 1) {
+  if (pl.ok && (pl.gb == 0 || (n + pl.gb - 1) / pl.gb == 1)) {
     // one scalar group: cl y-neighbour tiles (same z tile) form a thread-block cluster; the
     // tile count is padded to whole clusters (the extra blocks exit at once)
-    constexpr int ZB = 32 * NK;
-    const int nzt = (h->nz + ZB - 1) / ZB, nyt = (h->ny + pl.ty - 1) / pl.ty;
+    const int nzt = scalar_z_tiles(h->nz, NK, h->colgroup, h->nz % NK != 0), nyt = (h->ny + pl.ty - 1) / pl.ty;
     pl.cl = std::max(1, std::min(h->cluster > 0 ? h->cluster : kDefaultClusterScalars, nyt));
     pl.tiles = (nyt + pl.cl - 1) / pl.cl * pl.cl * nzt;
   }
@@ -490,7 +518,7 @@ template <typename T>
 const TensorMaps *field_maps(monc_adv_t h, const T *u, const T *v, const T *w, const void *const *q, int n,
                              int ty) {
   std::vector<const void *> ptrs = {u, v, w};
-  for (int s = 0; s < n; ++s) ptrs.push_back(q[s]);
+  for (int s = 0; s < n; ++s) ptrs.push_back(q[s]);  // (n = 0: q may be NULL)
   for (MapEntry &e : h->map_cache)
     if (e.ty == ty && e.ptrs == ptrs) {
       e.stamp = ++h->map_clock;
@@ -509,7 +537,7 @@ const TensorMaps *field_maps(monc_adv_t h, const T *u, const T *v, const T *w, c
   const int RS = kRowBytes / (int)sizeof(T);
   bool ok = true;
   for (int f = 0; f < 3 + kMaxScalarsPerLaunch; ++f) {
-    const void *base = f < 3 + n ? ptrs[f] : ptrs[3];
+    const void *base = f < 3 + n ? ptrs[f] : ptrs[n > 0 ? 3 : 0];
     ok = ok && encode_field_map<T>(h, &slot->maps.m[f], base, RS, ty + 2);
   }
   if (!ok) {
@@ -523,14 +551,14 @@ const TensorMaps *field_maps(monc_adv_t h, const T *u, const T *v, const T *w, c
   return &slot->maps;
 }
 
-template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false>
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false, bool RAG = false>
 int launch_tma_scalars_k(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
                          const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
-  CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>));
+  CU(allow_max_smem(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS, RAG>));
   dim3 grid(pl.tiles, pl.nchunks);
   const int threads = (pl.ty * (pl.ss + (MOM ? 1 : 0)) + 1) * 32;  // consumers + the producer warp
-  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS>, grid, pl.cl, threads, pl.smem, st, p, maps, outs, mo, nq,
-                (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz, pl.cl));
+  CU(launch_pdl(h, tma_scalars<T, GW, ACC, SKEW, MOM, WS, RAG>, grid, pl.cl, threads, pl.smem, st, p, maps, outs, mo, nq,
+                pl.gb == 0 ? 1 : (nq + pl.gb - 1) / pl.gb, pl.gb, pl.ty, pl.ss, pl.stages, pl.fieldsz, pl.cl));
   return MONC_ADV_OK;
 }
 
@@ -538,6 +566,16 @@ template <typename T, int GW, bool MOM>
 int launch_tma_scalars_m(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps, const SqPtrs<T> &outs,
                          const MomPtrs<T> &mo, int nq, const TmaScalarPlan &pl, cudaStream_t st) {
   const bool skew = h->form == MONC_ADV_FORM_PW_SKEW;
+  if (h->nz % VecOf<T>::NK != 0) {
+    // ragged nz: the RAG instantiations (levels shifted against the vectors, neighbour rows
+    // read element by element)
+    if (h->work > 1) return fail(h, MONC_ADV_EINVAL, "work scaling needs nz to be a whole number of 16-byte vectors");
+    if (h->accumulate)
+      return skew ? launch_tma_scalars_k<T, GW, true, true, MOM, false, true>(h, p, maps, outs, mo, nq, pl, st)
+                  : launch_tma_scalars_k<T, GW, true, false, MOM, false, true>(h, p, maps, outs, mo, nq, pl, st);
+    return skew ? launch_tma_scalars_k<T, GW, false, true, MOM, false, true>(h, p, maps, outs, mo, nq, pl, st)
+                : launch_tma_scalars_k<T, GW, false, false, MOM, false, true>(h, p, maps, outs, mo, nq, pl, st);
+  }
   if (h->work > 1)  // checked by work_scale_ok: flux form, overwrite
     return launch_tma_scalars_k<T, GW, false, false, MOM, true>(h, p, maps, outs, mo, nq, pl, st);
   if (h->accumulate)
@@ -561,21 +599,23 @@ int launch_tma_scalars(monc_adv_t h, const KParams<T> &p, const TensorMaps &maps
 template <typename T>
 int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T *w,
                     const void *const *q, void *const *sq, int nq, int ia, int ib,
-                    cudaStream_t st, bool *done, const MomPtrs<T> *mo = nullptr) {
+                    cudaStream_t st, bool *done, const MomPtrs<T> *mo) {
   *done = false;
   if (mo && nq > 10) return MONC_ADV_OK;
-  for (int base = 0; base < nq; base += kMaxScalarsPerLaunch) {
+  if (nq == 0 && !mo) return MONC_ADV_OK;
+  // (nq = 0 with mo: one launch of the momentum role alone)
+  for (int base = 0; base < std::max(nq, 1); base += kMaxScalarsPerLaunch) {
     const int n = std::min(kMaxScalarsPerLaunch, nq - base);
     const TmaScalarPlan &pl = plan_tma_scalars<T>(h, ib - ia, n, mo != nullptr);
     if (!pl.ok) {
       if (base == 0) return MONC_ADV_OK;
       return fail(h, MONC_ADV_ECUDA, "scalars: TMA plan failed after a partial launch");
     }
-    const TensorMaps *mp = field_maps<T>(h, u, v, w, q + base, n, pl.ty);
+    const TensorMaps *mp = field_maps<T>(h, u, v, w, n > 0 ? q + base : nullptr, n, pl.ty);
     if (!mp) return fail(h, MONC_ADV_ECUDA, "scalars: cuTensorMapEncodeTiled failed");
     const TensorMaps &maps = *mp;
     SqPtrs<T> outs;
-    for (int s = 0; s < kMaxScalarsPerLaunch; ++s) outs.sq[s] = (T *)sq[base + (s < n ? s : 0)];
+    for (int s = 0; s < kMaxScalarsPerLaunch; ++s) outs.sq[s] = n > 0 ? (T *)sq[base + (s < n ? s : 0)] : nullptr;
     p.xc = pl.xc;
     int rc = MONC_ADV_OK;
     switch (pl.gw) {
@@ -590,8 +630,10 @@ int run_tma_scalars(monc_adv_t h, KParams<T> p, const T *u, const T *v, const T 
     h->launches++;
     char b[200];
     snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d stages=%d xc=%d grid=%dx%d cluster=%d "
-             "threads=%d smem=%zu", mo ? "tma_fused(momentum+scalars)" : "tma_scalars", pl.gb, pl.gw, pl.ss,
-             pl.ty, pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.cl, (pl.ty * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
+             "colgroup=%d threads=%d smem=%zu",
+             mo ? (n > 0 ? "tma_fused(momentum+scalars)" : "tma_fused(momentum role only)") : "tma_scalars", pl.gb,
+             pl.gw, pl.ss, pl.ty, pl.stages, pl.xc, pl.tiles, pl.nchunks, pl.cl, std::max(1, h->colgroup),
+             (pl.ty * (pl.ss + (mo ? 1 : 0)) + 1) * 32, pl.smem);
     h->plan_sca = b;
     if (mo) h->plan_mom.clear();
   }
@@ -886,6 +928,11 @@ int monc_adv_create(monc_adv_t *out, int nx, int ny, int nz, int halo, double dx
   h->dx = dx; h->dy = dy;
   h->elems = (size_t)h->nxh * h->nyh * nz;
   h->esize = dtype == MONC_ADV_F64 ? 8 : 4;
+  {
+    int g = 1;
+    while (((size_t)g * nz * h->esize) % 16 != 0) g *= 2;  // 1, 2 or 4
+    h->colgroup = h->nyh % g == 0 ? g : 0;
+  }
   auto cfail = [&](cudaError_t e, const char *what) {
     g_create_error = std::string(what) + ": " + cudaGetErrorString(e);
     const int code = e == cudaErrorMemoryAllocation ? MONC_ADV_ENOMEM : MONC_ADV_ECUDA;
@@ -922,8 +969,12 @@ int monc_adv_create(monc_adv_t *out, int nx, int ny, int nz, int halo, double dx
   h->tz_host[0][0] = h->tz_host[1][0] = h->tz_host[2][0] = h->tz_host[3][0] = 0.0;
   h->tz_host[1][nz - 1] = 0.0;
   h->tz_host[2][nz - 1] = h->tz_host[3][nz - 1] = 0.0;
+  // device tables: zero-padded to whole 16-byte vectors plus one (the last thread of a ragged
+  // column reads its whole vector)
+  const size_t tz_bytes = ((size_t)nz * h->esize + 15) / 16 * 16 + 16;
   for (int a = 0; a < 4; ++a) {
-    e = cudaMalloc(&h->d_tz[a], (size_t)nz * h->esize);
+    e = cudaMalloc(&h->d_tz[a], tz_bytes);
+    if (e == cudaSuccess) e = cudaMemset(h->d_tz[a], 0, tz_bytes);
     if (e != cudaSuccess) return cfail(e, "cudaMalloc(constants)");
     if (dtype == MONC_ADV_F64) {
       e = cudaMemcpy(h->d_tz[a], h->tz_host[a].data(), (size_t)nz * 8, cudaMemcpyHostToDevice);
@@ -1214,10 +1265,12 @@ int monc_adv_set_variant(monc_adv_t h, int variant) {
   if (variant < 0 || variant > 3) return fail(h, MONC_ADV_EINVAL, "set_variant: 0..3");
   if (h->work > 1 && variant != 0 && variant != 3)
     return fail(h, MONC_ADV_EINVAL, "set_variant: work scaling is on (TMA kernels only)");
-  if (variant >= 2) {
-    const int nk = h->dtype == MONC_ADV_F64 ? 2 : 4;
-    if (h->nz % nk != 0) return fail(h, MONC_ADV_EINVAL, "set_variant: marching kernels need nz % (16/sizeof(dtype)) == 0");
-  }
+  const int nk = h->dtype == MONC_ADV_F64 ? 2 : 4;
+  if (variant == 2 && h->nz % nk != 0)
+    return fail(h, MONC_ADV_EINVAL, "set_variant: the direct-load marching kernels need nz % (16/sizeof(dtype)) == 0");
+  if (variant == 3 && h->colgroup == 0)
+    return fail(h, MONC_ADV_EINVAL, "set_variant: ragged nz needs ny + 2 halo to be a multiple of 2 (fp64, "
+                                    "fp32 with even nz) or 4 (fp32 with odd nz) for the TMA kernels");
   h->variant = variant;
   return MONC_ADV_OK;
 }

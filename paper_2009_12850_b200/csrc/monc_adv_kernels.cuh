@@ -40,6 +40,7 @@ struct KParams {
   long long plane;  // nyh * nz elements
   int ia, ib;       // output x range [ia, ib), array indices
   int xc;           // x planes marched per block
+  int colgroup;     // tma_scalars: columns per row of the tensor view (1; 2 or 4 when nz is ragged)
   int wzc;          // warps (z chunks of 32 vectors) per column
   int units;        // ny * wzc
   int accumulate;   // 0: overwrite, 1: add into outputs
@@ -48,7 +49,7 @@ struct KParams {
   int work;         // TMA kernels, WS instantiations: evaluations of the flux arithmetic per point
   T zero;           // 0, as a run-time value: x + zero * r is x, but no compiler can know it
   T cx, cy;         // 1/(4dx), 1/(4dy)
-  const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz; tzc2[nz-1] = 0
+  const T *tzc1, *tzc2, *tzd1, *tzd2;  // device tables, length nz padded with zeros to whole vectors + one; tzc2[nz-1] = 0
 };
 
 template <typename T>

@@ -162,6 +162,58 @@ __device__ __forceinline__ Vec<T> down_with(const Vec<T> &a, const T bot) {
   r.v[0] = bot;
   return r;
 }
+// Element-wise global access for the threads whose 16-byte vector is not whole or not
+// aligned in the caller's array (nz not a multiple of the vector: DESIGN.md 6.8)
+template <typename T>
+__device__ __forceinline__ void st_elems(T *p, const Vec<T> &a, const int nlo, const int nhi) {
+#pragma unroll
+  for (int e = 0; e < VecOf<T>::NK; ++e)
+    if (e >= nlo && e < nhi) __stcs(p + e, a.v[e]);
+}
+template <typename T>
+__device__ __forceinline__ Vec<T> ld_elems_rw(const T *p, const int nlo, const int nhi) {
+  Vec<T> r;
+#pragma unroll
+  for (int e = 0; e < VecOf<T>::NK; ++e) r.v[e] = (e >= nlo && e < nhi) ? p[e] : T(0);
+  return r;
+}
+// NK consecutive elements from an address that is element-aligned only (ragged nz: a
+// neighbour row's levels are not vector-aligned with the centre row's)
+__device__ __forceinline__ Vec<double> lds_elems(uint32_t a, const double *tag) {
+  Vec<double> r;
+  r.v[0] = lds1_at<0>(a, tag); r.v[1] = lds1_at<8>(a, tag);
+  return r;
+}
+__device__ __forceinline__ Vec<float> lds_elems(uint32_t a, const float *tag) {
+  Vec<float> r;
+  if ((a & 7u) == 0) {
+    // warp-uniform (the lanes are 16 bytes apart): two 8-byte loads are conflict-free at that
+    // stride, four 4-byte loads are 4-way bank conflicts each
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.v[0]), "=f"(r.v[1]) : "r"(a));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+8];" : "=f"(r.v[2]), "=f"(r.v[3]) : "r"(a));
+  } else {
+    r.v[0] = lds1_at<0>(a, tag); r.v[1] = lds1_at<4>(a, tag); r.v[2] = lds1_at<8>(a, tag); r.v[3] = lds1_at<12>(a, tag);
+  }
+  return r;
+}
+// a neighbour row's vector: one 16-byte load, or element by element when RAG
+template <bool RAG, typename T>
+__device__ __forceinline__ Vec<T> lds_row(uint32_t a, const T *tag) {
+  if constexpr (RAG) return lds_elems(a, tag);
+  else return lds_at<0>(a, tag);
+}
+// coefficient vector of levels k0 .. k0+NK-1; RAG: element by element, 0 outside the column
+template <bool RAG, typename T>
+__device__ __forceinline__ Vec<T> ld_coef(const T *tz, const int k0, const int nz) {
+  if constexpr (!RAG) {
+    return ld_vec(tz + k0);
+  } else {
+    Vec<T> r;
+#pragma unroll
+    for (int e = 0; e < VecOf<T>::NK; ++e) r.v[e] = (k0 + e >= 0 && k0 + e < nz) ? __ldg(tz + k0 + e) : T(0);
+    return r;
+  }
+}
 // x & m bit by bit (m = 0 or ~0): forces an exact +0 without a predicate, so the
 // "no tendency at this level" rule costs a logic op instead of a compare + select
 __device__ __forceinline__ double keep_if(double x, int m) {
@@ -192,24 +244,29 @@ __device__ __forceinline__ float keep_if(float x, int m) {
 template <typename T>
 struct MarchArgs {
   uint32_t a0, fb, sbytes, rsb, bar0;
+  uint32_t rsbS, rsbN;  // bytes back to the south row / on to the north row (rsb; shifted by whole elements when RAG)
   int nstages, nsteps, lane;
   int work;  // WS: evaluations of the arithmetic per step (results identical)
   T zero;    // WS: 0 as a run-time value (same_value)
   bool act, bot_edge;
-  bool first_level, last_level;  // element 0 is level K = 1 (no tendency) / element NK-1 is level K = nz (sw = 0)
+  bool vst;        // all NK levels of the thread's vector exist (it is 16-byte aligned by construction)
+  int nlo, nhi;    // elements [nlo, nhi) of the vector are levels of the column (0, NK unless nz is ragged)
+  int first_elem;  // element that is level K = 1 (no tendency), -1 if none
+  int last_elem;   // element that is level K = nz (sw = 0), -1 if none
   T *su, *sv, *sw;            // output arrays (kernel parameters: re-read from the constant bank, not kept in registers)
   long long c0, plane;        // element offset of (i0, j, k0); elements per x plane
   T cx, cy;
   Vec<T> c1, c2, d1, d2;
 };
 
-template <typename T, bool ACC, bool SKEW, bool WS, typename AfterRelease>
+template <typename T, bool ACC, bool SKEW, bool WS, bool RAG, typename AfterRelease>
 __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelease &&after_release) {
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
   constexpr int UP = NK * SZ;  // byte offset of the level above a vector's last element
   const T *const tag = nullptr;
-  const uint32_t a0 = m.a0, fb = m.fb, sbytes = m.sbytes, rsb = m.rsb, bar0 = m.bar0;
+  const uint32_t a0 = m.a0, fb = m.fb, sbytes = m.sbytes, bar0 = m.bar0;
+  const uint32_t rsbS = RAG ? m.rsbS : m.rsb, rsbN = RAG ? m.rsbN : m.rsb;
   const int nstages = m.nstages, lane = m.lane;
   const bool bot_edge = m.bot_edge;
   long long c = m.c0;
@@ -219,7 +276,7 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
   XFlux<T> FA, FB;
   RA.u = lds_at<0>(a0, tag);
   RA.v = lds_at<0>(a0 + fb, tag);
-  RA.vs = lds_at<0>(a0 + fb - rsb, tag);
+  RA.vs = lds_row<RAG>(a0 + fb - rsbS, tag);
   RA.w = lds_at<0>(a0 + 2 * fb, tag);
 #pragma unroll
   for (int e = 0; e < NK; ++e) FA.xx.v[e] = FA.xy.v[e] = FA.xz.v[e] = T(0);
@@ -238,25 +295,31 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
     if (ACC) {
 #pragma unroll
       for (int e = 0; e < NK; ++e) au.v[e] = av.v[e] = aw.v[e] = T(0);
-      if (!first && m.act) { au = ld_vec_rw(m.su + c); av = ld_vec_rw(m.sv + c); aw = ld_vec_rw(m.sw + c); }
+      if (!first) {
+        if (m.vst) { au = ld_vec_rw(m.su + c); av = ld_vec_rw(m.sv + c); aw = ld_vec_rw(m.sw + c); }
+        else if (RAG && m.act) {
+          au = ld_elems_rw(m.su + c, m.nlo, m.nhi); av = ld_elems_rw(m.sv + c, m.nlo, m.nhi);
+          aw = ld_elems_rw(m.sw + c, m.nlo, m.nhi);
+        }
+      }
     }
     mbar_wait(bar0 + 8 * sE, parE);  // plane i+1 has landed
     chk_jitter(1);
     const uint32_t pCv = pC + fb, pCw = pCv + fb, pEv = pE + fb;
-    const Vec<T> uS = lds_at<0>(pC - rsb, tag), uN = lds_at<0>(pC + rsb, tag);
-    const Vec<T> vN = lds_at<0>(pCv + rsb, tag);
-    const Vec<T> wS = lds_at<0>(pCw - rsb, tag), wN = lds_at<0>(pCw + rsb, tag);
+    const Vec<T> uS = lds_row<RAG>(pC - rsbS, tag), uN = lds_row<RAG>(pC + rsbN, tag);
+    const Vec<T> vN = lds_row<RAG>(pCv + rsbN, tag);
+    const Vec<T> wS = lds_row<RAG>(pCw - rsbS, tag), wN = lds_row<RAG>(pCw + rsbN, tag);
     RE.u = lds_at<0>(pE, tag);
     RE.v = lds_at<0>(pEv, tag);
-    RE.vs = lds_at<0>(pEv - rsb, tag);
+    RE.vs = lds_row<RAG>(pEv - rsbS, tag);
     RE.w = lds_at<0>(pEv + fb, tag);
     const Vec<T> uCu = up_with(RC.u, lds1_at<UP>(pC, tag)), vCu = up_with(RC.v, lds1_at<UP>(pCv, tag));
     const Vec<T> wCu = up_with(RC.w, lds1_at<UP>(pCw, tag));
-    const Vec<T> vSu = up_with(RC.vs, lds1_at<UP>(pCv - rsb, tag));
+    const Vec<T> vSu = up_with(RC.vs, lds1_at<UP>(pCv - rsbS, tag));
     T b_xz = T(0), b_yz = T(0), b_zz = T(0);
     if (bot_edge) {  // the level below this warp's first: fluxes a shuffle cannot provide
       const T ub = lds1_at<-SZ>(pC, tag), vb = lds1_at<-SZ>(pCv, tag), wb = lds1_at<-SZ>(pCw, tag);
-      const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + rsb, tag);
+      const T web = lds1_at<-SZ>(pEv + fb, tag), wnb = lds1_at<-SZ>(pCw + rsbN, tag);
       if (SKEW) {
         b_xz = ub * (wb + web);
         b_yz = vb * (wb + wnb);
@@ -290,15 +353,26 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + sC));
     if (!first) {
       after_release();
-      if (m.first_level) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
-      if (m.last_level) ow.v[NK - 1] = T(0);
+      if (RAG) {
+        if (m.first_elem >= 0 || m.last_elem >= 0) {
+#pragma unroll
+          for (int e = 0; e < NK; ++e) {
+            if (e == m.first_elem) { ou.v[e] = T(0); ov.v[e] = T(0); ow.v[e] = T(0); }
+            if (e == m.last_elem) ow.v[e] = T(0);
+          }
+        }
+      } else {
+        if (m.first_elem == 0) { ou.v[0] = T(0); ov.v[0] = T(0); ow.v[0] = T(0); }
+        if (m.last_elem == NK - 1) ow.v[NK - 1] = T(0);
+      }
       if (m.act) {
         T *qu = m.su + c, *qv = m.sv + c, *qw = m.sw + c;
         if (ACC) {
 #pragma unroll
           for (int e = 0; e < NK; ++e) { ou.v[e] += au.v[e]; ov.v[e] += av.v[e]; ow.v[e] += aw.v[e]; }
         }
-        st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow);
+        if (!RAG || m.vst) { st_vec(qu, ou); st_vec(qv, ov); st_vec(qw, ow); }
+        else { st_elems(qu, ou, m.nlo, m.nhi); st_elems(qv, ov, m.nlo, m.nhi); st_elems(qw, ow, m.nlo, m.nhi); }
       }
       c += m.plane;
     }
@@ -408,13 +482,15 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   m.nstages = nstages; m.nsteps = nsteps; m.lane = lane;
   m.work = p.work; m.zero = p.zero;
   m.bot_edge = m.act && lane == 0 && zc > 0;
-  m.first_level = k0 == 0;
-  m.last_level = k0 + NK == nz;
+  m.vst = m.act; m.nlo = 0; m.nhi = NK;  // this kernel takes whole, aligned vectors only (nz % NK == 0)
+  m.first_elem = k0 == 0 ? 0 : -1;
+  m.last_elem = (k0 + NK == nz) ? NK - 1 : -1;
+  m.rsbS = m.rsbN = (uint32_t)(nz * SZ);
   m.c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
   m.su = su; m.sv = sv; m.sw = sw;
   m.plane = p.plane;
   m.cx = p.cx; m.cy = p.cy;
-  momentum_march<T, ACC, SKEW, WS>(m, [&]() {
+  momentum_march<T, ACC, SKEW, WS, false>(m, [&]() {
     if (producer && to_issue > 0) {
       // slot of plane i-1: every warp released it during the previous step
       mbar_wait(bar0 + 8 * (nstages + s_next), par_next);
@@ -502,22 +578,41 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
 constexpr int kScalarConsumerWarps = 15;
 constexpr int kScalarThreads = (kScalarConsumerWarps + 1) * 32;
 constexpr int kRowBytes = 34 * 16;  // 32 vectors of the tile + one vector of z halo on each side
+// Ragged nz (tma_scalars, RAG): the tensor view holds G columns per row; the columns j = c mod G
+// of a tile ("class" c) are one box of ceil(rows / G) box rows, staged in a class block of its
+// own (128-byte aligned: a tensor copy's destination must be): bytes of one class block / field
+__host__ __device__ constexpr int ragged_class_rows(int rows, int g) { return (rows + g - 1) / g; }
+__host__ __device__ constexpr int ragged_class_bytes(int rows, int g) {
+  return (ragged_class_rows(rows, g) * kRowBytes + 127) / 128 * 128;
+}
+// bytes of one field tile of `rows` rows in a ring stage
+__host__ __device__ constexpr int scalar_field_bytes(int rows, int g, bool rag) {
+  return rag ? g * ragged_class_bytes(rows, g) : (rows * kRowBytes + 127) / 128 * 128;
+}
+// z tiles of 32 vectors per column; a ragged column's levels are shifted by up to NK-1
+// elements against its vectors (tma_scalars, RAG)
+__host__ __device__ constexpr int scalar_z_tiles(int nz, int nk, int g, bool rag) {
+  int shift = 0;  // the largest (c nz) mod NK over the classes c < G
+  if (rag)
+    for (int c = 1; c < g; ++c) shift = (c * (nz % nk)) % nk > shift ? (c * (nz % nk)) % nk : shift;
+  return (nz + shift + 32 * nk - 1) / (32 * nk);
+}
 
 // The scalar role of one warp: GW scalars (mycnt of them live when !FULL) of one
 // column chunk over the block's planes.
-template <typename T, int GW, bool ACC, bool SKEW, bool FULL, bool WS>
+template <typename T, int GW, bool ACC, bool SKEW, bool FULL, bool WS, bool RAG>
 __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t fb, const uint32_t sbytes,
-                                             const uint32_t q0off, const uint32_t bar0, const int nstages,
+                                             const uint32_t rsbS, const uint32_t rsbN, const uint32_t q0off, const uint32_t bar0, const int nstages,
                                              const int nplanes, const int mycnt, const int work, const T zero,
                                              const int lane,
-                                             const bool act, const bool bot_edge, const int keep_first,
+                                             const bool act, const bool vst, const int nlo, const int nhi,
+                                             const bool bot_edge, const int (&keep)[VecOf<T>::NK],
                                              T *const *__restrict__ sqp, const long long c0,
                                              const long long plane, const Vec<T> &c1, const Vec<T> &c2,
                                              const T cx2, const T cy2) {
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
   constexpr int UP = NK * SZ;
-  constexpr int RSB = kRowBytes;
   const T *const tag = nullptr;
   // carried per scalar: q of the previous plane (two register sets that swap roles in
   // the x loop unrolled by two, so the rotation costs no moves) and A = P + f of it
@@ -539,7 +634,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
     mbar_wait(bar0 + 8 * st, par);  // the next plane has landed
     chk_jitter(4);
     const uint32_t pV = pA + fb, pW = pV + fb;
-    Vec<T> vs = lds_at<-RSB>(pV, tag), vn = lds_at<0>(pV, tag);
+    Vec<T> vs = lds_row<RAG>(pV - rsbS, tag), vn = lds_at<0>(pV, tag);
     Vec<T> wt = lds_at<0>(pW, tag);
     Vec<T> wl = down_with(wt, lds1_at<-SZ>(pW, tag));  // w one level below each element
     un = lds_at<0>(pA, tag);  // read now: the slot's release must not wait for it
@@ -555,7 +650,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
       if (FULL || s < mycnt) {  // warp-uniform
         QN[s] = lds_at<0>(pQ, tag);
         const Vec<T> &q = QN[s];
-        const Vec<T> qS = lds_at<-RSB>(pQ, tag), qN = lds_at<RSB>(pQ, tag);
+        const Vec<T> qS = lds_row<RAG>(pQ - rsbS, tag), qN = lds_row<RAG>(pQ + rsbN, tag);
         const T qtop = lds1_at<UP>(pQ, tag);  // the level above the thread's last
         // the level below the thread's first: lane 0 reads it, the others get it by shuffle
         const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
@@ -609,16 +704,26 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
         }
         CA[s] = can;
         if (STORE) {  // sq of the previous plane is complete
-          o.v[0] = keep_if(o.v[0], keep_first);
+          if (RAG) {  // level K = 1 may be any element of the vector
+#pragma unroll
+            for (int e = 0; e < NK; ++e) o.v[e] = keep_if(o.v[e], keep[e]);
+          } else {
+            o.v[0] = keep_if(o.v[0], keep[0]);
+          }
           T *sq = sqp[s] + c;  // pointer table lives in the constant bank
           if (ACC) {
             if (act) {
-              const Vec<T> a = ld_vec_rw(sq);
+              const Vec<T> a = (!RAG || vst) ? ld_vec_rw(sq) : ld_elems_rw(sq, nlo, nhi);
 #pragma unroll
               for (int e = 0; e < NK; ++e) o.v[e] += a.v[e];
             }
           }
-          if (act) st_vec(sq, o);  // nothing but the store under the predicate
+          if (RAG) {
+            if (vst) st_vec(sq, o);
+            else if (act) st_elems(sq, o, nlo, nhi);  // a vector that straddles an end of the column
+          } else {
+            if (act) st_vec(sq, o);  // nothing but the store under the predicate
+          }
         }
         pQ += fb;
       }
@@ -645,7 +750,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
   }
 }
 
-template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false>
+template <typename T, int GW, bool ACC, bool SKEW, bool MOM, bool WS = false, bool RAG = false>
 __global__ void __launch_bounds__(kScalarThreads, 1)
 tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const SqPtrs<T> outs,
             const MomPtrs<T> mo, const int nq, const int ngroups, const int gb, const int ty,
@@ -653,7 +758,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   constexpr int NK = VecOf<T>::NK;
   constexpr int SZ = (int)sizeof(T);
   constexpr int ZB = 32 * NK;                // levels per block tile
-  constexpr int RS = kRowBytes / SZ;         // row stride in elements
+  constexpr uint32_t rowb = (uint32_t)kRowBytes;  // bytes between consecutive rows of a tile (of a class block, RAG)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int nz = p.nz;
   const int lane = threadIdx.x & 31;
@@ -668,7 +773,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   // sharing a wind tile run together and the later reads hit L2
   const int grp = blockIdx.x % ngroups;
   const int tile = blockIdx.x / ngroups;
-  const int nzt = (nz + ZB - 1) / ZB;
+  const int nzt = scalar_z_tiles(nz, NK, p.colgroup, RAG);
   // `cl` consecutive blocks are one thread-block cluster: y-neighbour tiles of the same z
   // tile, co-scheduled on one GPC so that they advance at the same rate and find each
   // other's halo rows in L2 (cl = 1: z tile fastest).  Tiles past the last y tile pad the
@@ -704,10 +809,13 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     // ---------------- producer warp: one lane per field ----------------
     const int nfld = 3 + cnt;
     const uint32_t box_bytes = (uint32_t)(rows * kRowBytes);
-    const CUtensorMap *mymap = &maps.m[lane < 3 ? lane : 3 + s0 + min(lane - 3, cnt - 1)];
+    const CUtensorMap *mymap = &maps.m[lane < 3 ? lane : 3 + s0 + max(0, min(lane - 3, cnt - 1))];
     if (lane < nfld) prefetch_tensormap(mymap);
     pdl_wait();  // the fields may have been written by the previous kernel in the stream
     const uint32_t dst0 = t0 + (uint32_t)(lane * fieldsz * SZ);
+    const int G = p.colgroup;
+    const int jcfirst = jr0 + p.h - 1;  // array column of the tile's first row
+    const uint32_t cbs = (uint32_t)ragged_class_bytes(rows, G);
     int s = 0;
     uint32_t par = 1;  // a fresh mbarrier passes a wait on parity 1: the first lap does not block
 #pragma unroll 1
@@ -716,10 +824,27 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
       chk_jitter(6);
       if (n >= nstages) chk_poison(t0 + (uint32_t)(s * stagesz * SZ), (uint32_t)(stagesz * SZ), lane, 32);
       const uint32_t full = bar0 + 8 * s;
-      if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
-      __syncwarp();
-      if (lane < nfld)
-        tma_load_3d(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+      if constexpr (!RAG) {
+        if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
+        __syncwarp();
+        if (lane < nfld)
+          tma_load_3d(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+      } else {
+        // ragged nz (a column is not a whole number of 16-byte vectors): the descriptor views G
+        // columns as one row (G nz elements: a multiple of 16 bytes), so column j is the elements
+        // from (j mod G) nz of row j / G.  One copy per field and class c = j mod G brings that
+        // class's columns of the tile (consecutive rows of the view) into its class block.  A copy
+        // must start on a 16-byte boundary: it starts at the vector that holds level kb0 - NK of
+        // the column, i.e. the class is staged shifted by (c nz) mod NK elements (the consumers know).
+        if (lane == 0) mbar_expect_tx(full, (uint32_t)(nfld * G * ragged_class_rows(rows, G) * kRowBytes));
+        __syncwarp();
+        for (int idx = lane; idx < nfld * G; idx += 32) {
+          const int f = idx / G, c = idx - f * G;
+          const int e0 = c * nz;  // the column's first level in its row of the view
+          tma_load_3d(t0 + (uint32_t)((s * stagesz + f * fieldsz) * SZ) + (uint32_t)c * cbs,
+                      &maps.m[f < 3 ? f : s0 + f], e0 - e0 % NK + kb0 - NK, (jcfirst - c + G - 1) / G, i0 - 1 + n, full);
+        }
+      }
       if (++s == nstages) { s = 0; par ^= 1; }
     }
     return;
@@ -729,39 +854,68 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   const int col = warp / nr;
   const int sp = warp - col * nr;
   if (col >= ncol) return;
-  const int k0r = kb0 + lane * NK;
-  const bool act = k0r < nz;
-  const int k0 = act ? k0r : nz - NK;  // clamp: finite data, never stored
-  const bool bot_edge = act && lane == 0 && k0 > 0;
+  // RAG: column jc starts mc elements into a 16-byte vector of the array; its threads own the
+  // vectors of the ARRAY (so the centre row is vector-aligned in shared memory and the stores
+  // are vector-aligned in global memory), i.e. levels shifted down by mc; the neighbour rows
+  // are shifted by their own amounts and are read element by element
+  const int jc = jr0 + col + p.h;
+  const int mc = RAG ? (int)(((long long)jc * nz) % NK) : 0;
+  const int k0r = kb0 + lane * NK - mc;
+  const int nlo = max(0, -k0r), nhi = min(NK, nz - k0r);  // elements [nlo, nhi) are levels of the column
+  const bool act = nhi > nlo;
+  const int k0 = RAG ? k0r : (act ? k0r : kb0);  // !RAG: clamp (finite data, never stored)
+  const bool bot_edge = act && lane == 0 && k0r > 0;
   const uint32_t fb = (uint32_t)(fieldsz * SZ), sbytes = (uint32_t)(stagesz * SZ);
   // u(column, k0) in stage 0: row col+1 of the box, one vector of z halo before level kb0
-  const uint32_t a0 = t0 + (uint32_t)(((col + 1) * RS + (k0 - kb0 + NK)) * SZ);
+  uint32_t a0 = t0 + (uint32_t)(col + 1) * rowb + (uint32_t)((lane + 1) * NK * SZ);
+  uint32_t rsbS = rowb, rsbN = rowb;
+  if (RAG) {
+    // byte offset, in a field tile, of the row of array column j: class block j mod G, then the
+    // rows of that class in order; a row's levels sit (j nz) mod NK elements further on
+    const int G = p.colgroup, jcfirst = jr0 + p.h - 1;
+    const uint32_t cbs = (uint32_t)ragged_class_bytes(rows, G);
+    auto row_at = [&](const int j) {
+      const int c = j % G;
+      return (uint32_t)c * cbs + (uint32_t)(j / G - (jcfirst - c + G - 1) / G) * rowb;
+    };
+    const int mS = (int)(((long long)(jc - 1) * nz) % NK), mN = (int)(((long long)(jc + 1) * nz) % NK);
+    const uint32_t rc = row_at(jc);
+    a0 = t0 + rc + (uint32_t)((lane + 1) * NK * SZ);
+    rsbS = rc - row_at(jc - 1) - (uint32_t)((mS - mc) * SZ);
+    rsbN = row_at(jc + 1) - rc + (uint32_t)((mN - mc) * SZ);
+  }
   const long long c0 = ((long long)i0 * p.nyh + (jr0 + col + p.h)) * nz + k0;  // (i0, j, k0)
-  int keep_first = k0 == 0 ? 0 : -1;  // element 0 is level K = 1: no tendency
-  asm volatile("" : "+r"(keep_first));  // keep it a mask for a logic op: no compare + select per store
+  const bool vst = nlo == 0 && nhi == NK;  // all NK levels exist
+  int keep[NK];  // 0 for the element that is level K = 1 (no tendency), else ~0
+#pragma unroll
+  for (int e = 0; e < NK; ++e) {
+    keep[e] = k0r + e == 0 ? 0 : -1;
+    asm volatile("" : "+r"(keep[e]));  // keep it a mask for a logic op: no compare + select per store
+  }
   if (MOM && sp == ss) {
     // ---------------- momentum role (fused launch): su, sv, sw of this column chunk
     // from the wind tiles the scalar warps use
     MarchArgs<T> m;
-    m.c1 = ld_vec(p.tzc1 + k0); m.c2 = ld_vec(p.tzc2 + k0);
-    m.d1 = ld_vec(p.tzd1 + k0); m.d2 = ld_vec(p.tzd2 + k0);
-    m.a0 = a0; m.fb = fb; m.sbytes = sbytes; m.rsb = (uint32_t)kRowBytes; m.bar0 = bar0;
+    m.c1 = ld_coef<RAG>(p.tzc1, k0, nz); m.c2 = ld_coef<RAG>(p.tzc2, k0, nz);
+    m.d1 = ld_coef<RAG>(p.tzd1, k0, nz); m.d2 = ld_coef<RAG>(p.tzd2, k0, nz);
+    m.a0 = a0; m.fb = fb; m.sbytes = sbytes; m.rsb = rowb; m.rsbS = rsbS; m.rsbN = rsbN; m.bar0 = bar0;
     m.nstages = nstages; m.nsteps = nplanes - 1; m.lane = lane;
     m.work = p.work; m.zero = p.zero;
     m.act = act; m.bot_edge = bot_edge;
-    m.first_level = k0 == 0;
-    m.last_level = k0 + NK == nz;
+    m.vst = vst; m.nlo = nlo; m.nhi = nhi;
+    m.first_elem = (-k0r >= 0 && -k0r < NK) ? -k0r : -1;
+    m.last_elem = (nz - 1 - k0r >= 0 && nz - 1 - k0r < NK) ? nz - 1 - k0r : -1;
     m.su = mo.su; m.sv = mo.sv; m.sw = mo.sw;
     m.c0 = c0; m.plane = p.plane;
     m.cx = p.cx; m.cy = p.cy;
     pdl_wait();
-    momentum_march<T, ACC, SKEW, WS>(m, []() {});
+    momentum_march<T, ACC, SKEW, WS, RAG>(m, []() {});
     return;
   }
   if (sp >= slive) return;
   const int sb = sp * GW;              // first scalar (within the block's group) of this warp
   const int mycnt = min(GW, cnt - sb);
-  Vec<T> c1 = ld_vec(p.tzc1 + k0), c2 = ld_vec(p.tzc2 + k0);
+  Vec<T> c1 = ld_coef<RAG>(p.tzc1, k0, nz), c2 = ld_coef<RAG>(p.tzc2, k0, nz);
 #pragma unroll
   for (int e = 0; e < NK; ++e) { c1.v[e] *= T(2); c2.v[e] *= T(2); }
   const T cx2 = T(2) * p.cx, cy2 = T(2) * p.cy;
@@ -769,11 +923,13 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
   T *const *sqp = outs.sq + (s0 + sb);
   pdl_wait();  // accumulate mode reads sq, which the previous kernel may have written
   if (mycnt == GW)
-    scalar_march<T, GW, ACC, SKEW, true, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, p.zero,
-                                             lane, act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, true, WS, RAG>(a0, fb, sbytes, rsbS, rsbN, q0off, bar0, nstages, nplanes, mycnt,
+                                                  p.work, p.zero, lane, act, vst, nlo, nhi, bot_edge, keep, sqp, c0,
+                                                  p.plane, c1, c2, cx2, cy2);
   else
-    scalar_march<T, GW, ACC, SKEW, false, WS>(a0, fb, sbytes, q0off, bar0, nstages, nplanes, mycnt, p.work, p.zero,
-                                              lane, act, bot_edge, keep_first, sqp, c0, p.plane, c1, c2, cx2, cy2);
+    scalar_march<T, GW, ACC, SKEW, false, WS, RAG>(a0, fb, sbytes, rsbS, rsbN, q0off, bar0, nstages, nplanes, mycnt,
+                                                   p.work, p.zero, lane, act, vst, nlo, nhi, bot_edge, keep, sqp, c0,
+                                                   p.plane, c1, c2, cx2, cy2);
 }
 
 }  // namespace monc

@@ -123,6 +123,31 @@ def test_step_async_automatic_chunk_count():
     L.close()
 
 
+@pytest.mark.parametrize("nz,dtype", [(65, "f64"), (66, "f32"), (35, "f32")])
+def test_step_async_ragged_nz(nz, dtype):
+    # nz that is not a whole number of 16-byte vectors: the fused TMA launch per chunk all the same
+    cfg = gc.custom_cfg(18, 12, nz, nq=3, dtype=dtype, cid=406)
+    P, L = gc.make_pair(cfg)
+    L.set_variant("tma")
+    L.set_chunks(4)
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    names = synth.field_names(cfg)
+    Q = [synth.field(cfg, n) for n in names]
+    hin = [pinned(a, L) for a in (U, V, W)]
+    hq = [pinned(a, L) for a in Q]
+    hout, hsq = pinned_out(L, 3), pinned_out(L, 3)
+    L.step_async(*hin, hq, *hout, hsq)
+    L.step_wait()
+    assert "tma_fused" in L.describe_plan()
+    for o, w_, n in zip(hout, P.momentum(U, V, W), ("su", "sv", "sw")):
+        gc.check(cfg, o, w_, n)
+        gc.check_halo_untouched(cfg, o, n)
+    for o, q, n in zip(hsq, Q, names):
+        gc.check(cfg, o, P.scalar(U, V, W, q), n)
+        gc.check_halo_untouched(cfg, o, n)
+    L.close()
+
+
 def test_step_async_pw_skew():
     # the hybrid step in the PW-skew form (NEXT-1): x-slab launches of the TMA kernels
     cfg = gc.custom_cfg(24, 17, 128, nq=4, cid=403)

@@ -72,6 +72,13 @@ def test_checked_fused_ring(dtype, form):
     tp.run_tendencies(gc.custom_cfg(9, 5, 64, dtype=dtype, cid=621), 5, form=form, accumulate=True)
 
 
+def test_checked_ragged_nz():
+    # per-row copies of the column-group view (ragged nz): same ring, same protocol
+    for shape in (tp.RAGGED_NZ[1], tp.RAGGED_NZ[5]):
+        for _ in range(2):
+            tp.test_ragged_nz_on_the_tma_kernels(shape)
+
+
 def test_checked_hybrid_step():
     import test_gpu_async as ta
     for _ in range(REPS):

@@ -91,8 +91,8 @@ def test_config1_shape_fp32_and_scalars():
 # ragged / edge shapes: several tiles, partial warps, z-chunk edges, odd sizes
 # ---------------------------------------------------------------------------
 SHAPES = [
-    (13, 7, 38, 2),    # fp64 vectors ok, fp32 falls back to generic (38 % 4 != 0)
-    (9, 11, 37, 2),    # odd nz: generic kernels
+    (13, 7, 38, 2),    # fp64 vectors ok; fp32 ragged (38 % 4 != 0) and ny + 2h odd: generic kernels
+    (9, 11, 37, 2),    # odd nz and ny + 2h odd: generic kernels (the ragged-nz TMA path: RAGGED_NZ below)
     (10, 6, 70, 2),    # two z-chunks per column, ragged second chunk
     (6, 10, 160, 2),   # config 4's nz: 2.5 warps per column (fp64)
     (5, 9, 256, 1),    # halo 1, 4 z-chunks per column (fp64), 2 (fp32)
@@ -173,11 +173,11 @@ def test_P7_exact_through_gpu(dtype, variant):
     dz = np.array([1, 1, 2, 2, 4, 4], float)
     L = binding.MoncAdv(4, 4, 6, 2, 2.0, 4.0, dz, dz, np.array([1, 1, .5, .5, .25, .25]),
                         np.array([2, 1, 1, .5, .5, .25]), dtype=dtype)
-    if variant in ("march", "tma") and dtype == "f32":
+    if variant == "march" and dtype == "f32":
         with pytest.raises(binding.MoncAdvError):
-            L.set_variant(variant)  # nz = 6 is not a multiple of 4
+            L.set_variant(variant)  # nz = 6 is not a multiple of 4: no direct-load marching kernel
         return
-    L.set_variant(variant)
+    L.set_variant(variant)  # "tma" in fp32: nz = 6 is ragged, two columns per row of the tensor view
     # coefficient tables as the library stores them
     tz = dict(zip(("tzc1", "tzc2", "tzd1", "tzd2"), L.get_coefficients()))
     d = [gc.to_dev(a, L) for a in (U, V, W, Q)]
@@ -354,10 +354,88 @@ def test_user_supplied_tz_arrays_and_stream():
 
 
 # ---------------------------------------------------------------------------
+# ragged nz (a column is not a whole number of 16-byte vectors) on the TMA kernels:
+# the tensor-map view groups 2 or 4 columns per row, every row of a tile is its own
+# copy, stores of unaligned / partial vectors go element by element
+# ---------------------------------------------------------------------------
+RAGGED_NZ = [
+    (13, 8, 37, 2, "f64"),    # one z tile, partial last vector, columns alternate between aligned and not
+    (9, 14, 129, 2, "f64"),   # three z tiles, the last holds one level
+    (10, 6, 255, 1, "f64"),   # halo 1, four z tiles
+    (7, 10, 3, 2, "f64"),     # minimum nz
+    (13, 8, 38, 2, "f32"),    # nz % 4 = 2: two columns per row
+    (9, 8, 37, 2, "f32"),     # odd nz: four columns per row
+    (6, 12, 129, 2, "f32"),   # two z tiles, the last holds one level
+    (10, 6, 254, 1, "f32"),   # halo 1
+    (5, 4, 7, 2, "f32"),
+]
+
+
+@pytest.mark.parametrize("shape", RAGGED_NZ, ids=lambda s: "x".join(map(str, s)))
+def test_ragged_nz_on_the_tma_kernels(shape):
+    nx, ny, nz, h, dtype = shape
+    cfg = gc.custom_cfg(nx, ny, nz, halo=h, nq=4, dtype=dtype, cid=700 + nz)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    for form in ("flux", "pw_skew"):
+        skew = form == "pw_skew"
+        P, L = gc.make_pair(cfg)
+        L.set_variant("tma")  # no silent fall-back to the generic kernels
+        L.set_form(form)
+        D = [gc.to_dev(a, L) for a in H]
+        want = list(P.momentum(H[0], H[1], H[2], skew=skew)) + [P.scalar(H[0], H[1], H[2], q, skew=skew) for q in H[3:]]
+        for tuning in (dict(), dict(xchunk=4, tile_y=3, stages=3), dict(xchunk=3, tile_y=2, split=2)):
+            L.set_tuning(**tuning)
+            # momentum alone: the momentum role of the tensor-map kernel without scalar warps
+            outs = gc.fresh_out(L, 7)
+            L.momentum(D[0], D[1], D[2], *outs[:3])
+            assert "momentum role only" in L.describe_plan() and "colgroup=1 " not in L.describe_plan()
+            # scalars alone
+            L.scalars(D[3:], outs[3:])
+            assert "tma_scalars" in L.describe_plan()
+            torch.cuda.synchronize()
+            for o, w_, n in zip(outs, want, ["su", "sv", "sw"] + names[3:]):
+                gc.check(cfg, o, w_, n)
+                gc.check_halo_untouched(cfg, o, n)
+            # the whole step in one launch, then once more accumulating
+            outs2 = gc.fresh_out(L, 7)
+            L.tendencies(D[0], D[1], D[2], outs2[0], outs2[1], outs2[2], D[3:], outs2[3:])
+            assert "tma_fused(momentum+scalars)" in L.describe_plan()
+            torch.cuda.synchronize()
+            for a, b in zip(outs, outs2):
+                assert torch.equal(a, b)  # same arithmetic in both launches
+            L.set_accumulate(True)
+            L.tendencies(D[0], D[1], D[2], outs2[0], outs2[1], outs2[2], D[3:], outs2[3:])
+            L.momentum(D[0], D[1], D[2], *outs2[:3])
+            L.set_accumulate(False)
+            torch.cuda.synchronize()
+            for o, w_, n, m in zip(outs2, want, ["su", "sv", "sw"] + names[3:], (3, 3, 3, 2, 2, 2, 2)):
+                gc.check(cfg, o, m * w_, n + " accumulated")
+                gc.check_halo_untouched(cfg, o, n)
+        L.close()
+
+
+def test_ragged_nz_without_a_column_group_view_runs_the_generic_kernels():
+    # odd nz in fp64 needs ny + 2 halo even; otherwise the generic kernels run and the TMA variant is refused
+    cfg = gc.custom_cfg(9, 11, 37, dtype="f64", cid=720)
+    P, L = gc.make_pair(cfg)
+    with pytest.raises(binding.MoncAdvError) as e:
+        L.set_variant("tma")
+    assert e.value.code == binding.EINVAL
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    outs = gc.fresh_out(L, 3)
+    L.momentum(*[gc.to_dev(a, L) for a in (U, V, W)], *outs)
+    assert "generic_momentum" in L.describe_plan()
+    for o, w_, n in zip(outs, P.momentum(U, V, W), ("su", "sv", "sw")):
+        gc.check(cfg, o, w_, n)
+    L.close()
+
+
+# ---------------------------------------------------------------------------
 # guard bands: nothing outside the caller's arrays is read into a result or written
 # ---------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("variant", ["tma", "march", "generic"])
+@pytest.mark.parametrize("variant", ["tma", "march", "generic", "tma-ragged-nz"])
 @pytest.mark.parametrize("form", ["flux", "pw_skew"])
 def test_guard_bands(dtype, variant, form):
     """Every field sits inside a larger allocation whose guard regions hold NaN
@@ -366,7 +444,10 @@ def test_guard_bands(dtype, variant, form):
     past an output array changes its guard."""
     if variant == "march" and form == "pw_skew":
         pytest.skip("march kernels are flux-form only")
-    cfg = gc.custom_cfg(9, 10, 72, halo=1, nq=3, dtype=dtype, cid=307)
+    nz = 72
+    if variant == "tma-ragged-nz":  # the last column's top vector and the first column's z halo straddle the array ends
+        variant, nz = "tma", 71
+    cfg = gc.custom_cfg(9, 10, nz, halo=1, nq=3, dtype=dtype, cid=307)
     P, L = gc.make_pair(cfg)
     L.set_variant(variant)
     L.set_form(form)
