@@ -15,7 +15,7 @@ points advected per second over the K timed steps with inputs resident in HBM;
 SURVEY.md 8(a) a3).  The same line carries a >= 2 s `sustained` record of the
 headline step (the board reaches its power cap within a second), the two
 north_star calls timed kernel by kernel, and compact records of the other
-BASELINE configs (`other_configs`: config1 momentum only, config3 fp32, config4
+BASELINE configs (`other_configs`: config1 momentum only, config3 fp32 with its end-to-end step, a ragged-nz shape, config4
 the hybrid step from host memory).  Prints ONE JSON line (rank 0).
 
 --impl reference times the CPU oracle (oracle/, fp64, single thread) on the
@@ -456,8 +456,35 @@ def run_device_config(ctx, args, workload, cache, headline):
                                 "note": "kernel time with 16 x the arithmetic per byte; the hybrid step through the "
                                         "host link is timed at x16 in other_configs.config4 (PAPER.md:109)"}
     if not headline:
+        if cfg.dtype == "f32" and nq:
+            # the precision variant end to end (half the bytes on the host link)
+            del sets
+            gc.collect()
+            torch.cuda.empty_cache()
+            hin = [torch.empty(L.shape, dtype=tdt, pin_memory=True) for _ in names]
+            for t_, a in zip(hin, H):
+                t_.copy_(torch.from_numpy(a))
+            hout = [torch.zeros(L.shape, dtype=tdt, pin_memory=True) for _ in names]
+            L.set_chunks(args.chunks)
+            t_e2e = []
+            for _ in range(3):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+                L.step_wait()
+                t_e2e.append(time.perf_counter() - t0)
+            e_s = float(np.mean(t_e2e[1:]))
+            ph = L.step_times_ms()
+            plane_b = (cfg.ny + 2 * cfg.halo) * cfg.nz * es
+            rec["e2e"] = {"value": cfg.points / e_s / 1e9, "unit": "Gpts/s", "ms_per_step": e_s * 1e3, "steps": 2,
+                          "chunks": L.step_chunk_count(), "h2d_bytes_per_step": nf * (cfg.nx + 2) * plane_b,
+                          "d2h_bytes_per_step": nf * cfg.points * es,
+                          "h2d_GBs": nf * (cfg.nx + 2) * plane_b / (ph["h2d"] * 1e-3) / 1e9,
+                          "d2h_GBs": nf * cfg.points * es / (ph["d2h"] * 1e-3) / 1e9}
+            del hin, hout
+        else:
+            del sets
         L.close()
-        del sets
         gc.collect()
         torch.cuda.empty_cache()
         return rec
@@ -694,6 +721,43 @@ def run_hybrid_config(ctx, args, steps, warmup, with_cpu):
     return rec
 
 
+def run_ragged_nz(ctx, args):
+    """Config 2 with one level less (512x512x255 fp64, 3 + 10 fields): nz is not a whole number of
+    16-byte vectors, the shape round 1 sent to the one-thread-per-point kernels.  Timing only (device
+    random inputs; parity of this path: tests/test_gpu_parity.py::test_ragged_nz_on_the_tma_kernels)."""
+    torch = ctx.torch
+    from paper_2009_12850_b200 import binding, synth
+    nx, ny, nz, nq = 512, 512, 255, 10
+    g = synth.grid(nz)
+    out = {"config": {"workload": "config2 with nz = 255 (ragged)", "nx": nx, "ny": ny, "nz": nz, "nq": nq,
+                      "storage_dtype": "f64", "step_call": "monc_adv_tendencies", "data": "device randn (timing only)"}}
+    L = binding.MoncAdv(nx, ny, nz, 2, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"], dtype="f64")
+    gen = torch.Generator(device="cuda").manual_seed(20091285)
+    sets = [([torch.randn(L.shape, device="cuda", dtype=torch.float64, generator=gen) for _ in range(3 + nq)],
+             [torch.empty(L.shape, device="cuda", dtype=torch.float64) for _ in range(3 + nq)]) for _ in range(2)]
+    st = torch.cuda.Stream()
+    alg = bytes_fused(nq, "f64") * nx * ny * nz
+    peak, _ = peaks()
+
+    def step(i):
+        a, o = sets[i % 2]
+        L.tendencies(a[0], a[1], a[2], o[0], o[1], o[2], a[3:], o[3:], stream=st)
+
+    for variant in ("auto", "generic"):
+        L.set_variant(variant)
+        e0, e1 = timed_loop(ctx, st, step, 20, warm=3)
+        ctx.barrier()
+        ms = e0.elapsed_time(e1) / 20
+        out["tma_ragged" if variant == "auto" else "generic_kernels"] = {
+            "ms_per_step": ms, "value": nx * ny * nz / (ms * 1e-3) / 1e9, "algorithmic_GBs": alg / (ms * 1e-3) / 1e9,
+            "frac": alg / (ms * 1e-3) / 1e9 / peak, "launch_plan": L.describe_plan(), "steps": 20}
+    L.close()
+    del sets
+    gc.collect()
+    torch.cuda.empty_cache()
+    return out
+
+
 def compact(rec):
     """What a sub-record of `other_configs` keeps."""
     keep = ("value", "unit", "ms_per_step", "steps", "dtype", "gpu_launches", "launch_plan", "clocks",
@@ -705,7 +769,8 @@ def compact(rec):
     out["config"] = {k: rec["config"][k] for k in ("workload", "nx", "ny", "nz", "nq", "storage_dtype", "step_call")}
     if "e2e" in rec:
         e = rec["e2e"]
-        out["e2e"] = {k: e[k] for k in ("value", "ms_per_step", "chunks", "automatic_chunks", "h2d_GBs", "d2h_GBs",
+        out["e2e"] = {k: e[k] for k in ("value", "ms_per_step", "chunks", "automatic_chunks", "h2d_bytes_per_step",
+                                        "d2h_bytes_per_step", "h2d_GBs", "d2h_GBs",
                                         "link_alone_GBs", "overlap_ratio", "streaming_combine", "work_scale_16") if k in e}
     return out
 
@@ -736,6 +801,11 @@ def run_ours(args):
                     others[w] = compact(run_device_config(ctx, args, w, cache, headline=False))
             except Exception as e:  # a sub-record must not take the headline down with it
                 others[w] = {"error": f"{type(e).__name__}: {e}"}
+            if w == "config1":
+                try:
+                    others["ragged_nz"] = run_ragged_nz(ctx, args)
+                except Exception as e:
+                    others["ragged_nz"] = {"error": f"{type(e).__name__}: {e}"}
     if ctx.rank != 0:
         ctx.close()
         return

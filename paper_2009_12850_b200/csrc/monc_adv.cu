@@ -325,9 +325,6 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
   KParams<T> p = make_params<T>(h, ia, ib);
   TmaPlan pl;
   if (h->variant == 3 || h->variant == 0) pl = plan_tma<T>(h, ib - ia);
-  const bool ragged = h->nz % VecOf<T>::NK != 0 && h->colgroup > 1;  // served by the tensor-map kernel's momentum role
-  if (h->variant == 3 && !pl.ok && !ragged)
-    return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this nz / form");
   if (h->work > 1 && !pl.ok) return fail(h, MONC_ADV_EINVAL, "momentum: work scaling needs the TMA kernels");
   if (pl.ok) {
     p.xc = pl.xc;
@@ -346,32 +343,32 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
     snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d cluster=%d threads=%d smem=%zu", pl.ty,
              pl.stages, pl.xc, (int)grid.x, pl.nchunks, pl.cl, pl.ty * p.wzc * 32, pl.smem);
     h->plan_mom = b;
-  } else if (ragged && (h->variant == 0 || h->variant == 3)) {
-    // ragged nz: tma_momentum's 1-D bulk copies need whole vectors per column; the momentum
-    // role of the tensor-map kernel does not
-    bool done = false;
-    const MomPtrs<T> mo{su, sv, sw};
-    const int rc = run_tma_scalars<T>(h, p, u, v, w, nullptr, nullptr, 0, ia, ib, st, &done, &mo);
-    if (rc != MONC_ADV_OK) return rc;
-    if (done) return MONC_ADV_OK;
-    if (h->variant == 3) return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this shape");
-    h->plan_mom = "generic_momentum";
-    const long long n = (long long)(ib - ia) * h->ny * h->nz;
-    generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
-  } else if (use_march<T>(h)) {
-    const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
-    const int bx = (p.units + wpb - 1) / wpb;
-    p.xc = pick_xchunk(h, ib - ia, bx, 16 / wpb, 1);
-    dim3 grid(bx, (ib - ia + p.xc - 1) / p.xc);
-    if (p.wzc > 1)
-      march_momentum<T, true><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
-    else
-      march_momentum<T, false><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
-    h->plan_mom = "march_momentum xc=" + std::to_string(p.xc);
   } else {
-    h->plan_mom = "generic_momentum";
-    const long long n = (long long)(ib - ia) * h->ny * h->nz;
-    generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
+    if (h->colgroup >= 1 && (h->variant == 0 || h->variant == 3)) {
+      // tma_momentum's 1-D bulk copies need whole vectors per column and at most 16 warps per
+      // column; the momentum role of the tensor-map kernel, run without scalar warps, takes a
+      // ragged nz and columns of any height (z tiles)
+      bool done = false;
+      const MomPtrs<T> mo{su, sv, sw};
+      const int rc = run_tma_scalars<T>(h, p, u, v, w, nullptr, nullptr, 0, ia, ib, st, &done, &mo);
+      if (rc != MONC_ADV_OK || done) return rc;
+    }
+    if (h->variant == 3) return fail(h, MONC_ADV_EINVAL, "momentum: TMA variant does not fit this shape");
+    if (use_march<T>(h)) {
+      const int wpb = h->warps > 0 ? h->warps : kWarpsPerBlock;
+      const int bx = (p.units + wpb - 1) / wpb;
+      p.xc = pick_xchunk(h, ib - ia, bx, 16 / wpb, 1);
+      dim3 grid(bx, (ib - ia + p.xc - 1) / p.xc);
+      if (p.wzc > 1)
+        march_momentum<T, true><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+      else
+        march_momentum<T, false><<<grid, wpb * 32, 0, st>>>(p, u, v, w, su, sv, sw);
+      h->plan_mom = "march_momentum xc=" + std::to_string(p.xc);
+    } else {
+      h->plan_mom = "generic_momentum";
+      const long long n = (long long)(ib - ia) * h->ny * h->nz;
+      generic_momentum<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, u, v, w, su, sv, sw);
+    }
   }
   CU(cudaGetLastError());
   h->launches++;

@@ -415,6 +415,32 @@ def test_ragged_nz_on_the_tma_kernels(shape):
         L.close()
 
 
+@pytest.mark.parametrize("dtype,nz", [("f64", 1100), ("f32", 2200), ("f64", 1101)])
+def test_tall_columns_take_the_tensor_map_kernel(dtype, nz):
+    # more than 16 warps per column: tma_momentum (whole columns per block) does not fit, the z-tiled
+    # tensor-map kernel does, momentum alone included
+    cfg = gc.custom_cfg(5, 6, nz, nq=2, dtype=dtype, cid=730)
+    P, L = gc.make_pair(cfg)
+    L.set_variant("tma")
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    D = [gc.to_dev(a, L) for a in H]
+    want = list(P.momentum(H[0], H[1], H[2])) + [P.scalar(H[0], H[1], H[2], q) for q in H[3:]]
+    outs = gc.fresh_out(L, 5)
+    L.momentum(D[0], D[1], D[2], *outs[:3])
+    assert "momentum role only" in L.describe_plan()
+    L.scalars(D[3:], outs[3:])
+    outs2 = gc.fresh_out(L, 5)
+    L.tendencies(D[0], D[1], D[2], outs2[0], outs2[1], outs2[2], D[3:], outs2[3:])
+    assert "tma_fused(momentum+scalars)" in L.describe_plan()
+    torch.cuda.synchronize()
+    for o, o2, w_, n in zip(outs, outs2, want, ["su", "sv", "sw"] + names[3:]):
+        gc.check(cfg, o, w_, n)
+        gc.check_halo_untouched(cfg, o, n)
+        assert torch.equal(o, o2)
+    L.close()
+
+
 def test_ragged_nz_without_a_column_group_view_runs_the_generic_kernels():
     # odd nz in fp64 needs ny + 2 halo even; otherwise the generic kernels run and the TMA variant is refused
     cfg = gc.custom_cfg(9, 11, 37, dtype="f64", cid=720)
