@@ -41,6 +41,11 @@ int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int w
  * that re-read each other's halo rows running at the same rate. */
 int monc_adv_set_cluster(monc_adv_t h, int n);
 
+/* L2 eviction priority the TMA kernels ask for on their input copies: 1 (default)
+ * evict_last -- a tile's halo rows are read again by the neighbouring blocks a few
+ * steps later --, 0 no hint, 2 evict_first (for measurements). */
+int monc_adv_set_l2_hint(monc_adv_t h, int hint);
+
 /* 1 (default): the TMA kernels are launched with CUDA's programmatic
  * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
  * predecessor in the stream (it waits for the predecessor's completion before

@@ -33,7 +33,7 @@ SYMBOLS = [
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
     "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version", "monc_adv_set_work_scale",
-    "monc_adv_set_cluster",
+    "monc_adv_set_cluster", "monc_adv_set_l2_hint",
 ]
 
 
@@ -96,7 +96,7 @@ def load():
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
                  "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
-                 "monc_adv_set_fuse", "monc_adv_set_work_scale", "monc_adv_set_cluster"):
+                 "monc_adv_set_fuse", "monc_adv_set_work_scale", "monc_adv_set_cluster", "monc_adv_set_l2_hint"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -272,6 +272,9 @@ class MoncAdv:
 
     def set_pdl(self, on):
         self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
+
+    def set_l2_hint(self, hint):
+        self._check(self._lib.monc_adv_set_l2_hint(self._h, int(hint)))
 
     def set_cluster(self, n):
         self._check(self._lib.monc_adv_set_cluster(self._h, int(n)))

@@ -77,6 +77,7 @@ struct monc_adv_s {
   int xchunk = 0, group = 0, prefetch = 0, warps = 0;  // 0 = default
   int stages = 0, tile_y = 0, split = 0;                // TMA kernels, 0 = default
   int cluster = 0;                                      // TMA kernels: y tiles per thread-block cluster, 0 = default
+  int l2hint = 1;                                       // TMA kernels: input copies ask L2 to evict them last
   int smem_optin = 0;                                   // max dynamic smem per block
   long launches = 0;
   std::string err;
@@ -157,6 +158,7 @@ KParams<T> make_params(monc_adv_t h, int ia, int ib) {
   p.ia = ia; p.ib = ib;
   constexpr int NK = VecOf<T>::NK;
   p.colgroup = std::max(1, h->colgroup);
+  p.l2hint = h->l2hint;
   p.wzc = (h->nz / NK + 31) / 32;
   p.units = h->ny * p.wzc;
   p.xc = ib - ia;
@@ -1248,6 +1250,13 @@ int monc_adv_set_cluster(monc_adv_t h, int n) {
   h->cluster = n;
   h->mom_plans.clear();
   h->sca_plans.clear();
+  return MONC_ADV_OK;
+}
+
+int monc_adv_set_l2_hint(monc_adv_t h, int hint) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (hint < 0 || hint > 2) return fail(h, MONC_ADV_EINVAL, "set_l2_hint: 0 (none), 1 (evict_last) or 2 (evict_first)");
+  h->l2hint = hint;
   return MONC_ADV_OK;
 }
 

@@ -40,6 +40,7 @@ struct KParams {
   long long plane;  // nyh * nz elements
   int ia, ib;       // output x range [ia, ib), array indices
   int xc;           // x planes marched per block
+  int l2hint;       // TMA kernels: L2 eviction hint of the input copies (0 none, 1 evict_last, 2 evict_first)
   int colgroup;     // tma_scalars: columns per row of the tensor view (1; 2 or 4 when nz is ragged)
   int wzc;          // warps (z chunks of 32 vectors) per column
   int units;        // ny * wzc

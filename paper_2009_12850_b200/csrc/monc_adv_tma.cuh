@@ -66,6 +66,25 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void *src, uint3
       : "memory");
 }
 
+// the same copy with an L2 eviction-priority hint for the lines it reads
+__device__ __forceinline__ void tma_load_1d_hint(uint32_t dst, const void *src, uint32_t bytes,
+                                                 uint32_t bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+      ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+      : "memory");
+}
+// Input tiles are read by two to four blocks each (the halo rows and z-halo vectors of the
+// neighbouring tiles) at times that drift apart during a march: asking L2 to evict them last
+// keeps more of the re-reads out of DRAM (+1.7 % sustained on the fused config-2 launch;
+// evict_first costs 5-10 %: DESIGN.md 7.1).  0 = no hint.
+__device__ __forceinline__ uint64_t l2_policy(const int hint) {
+  uint64_t pol = 0;
+  if (hint == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  if (hint == 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+
 // Programmatic dependent launch (PDL): a kernel launched with the programmatic
 // stream-serialisation attribute may start while its predecessor in the stream
 // drains.  pdl_launch_dependents() lets the successor's blocks be scheduled as
@@ -458,15 +477,22 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   const uint32_t t0 = smem_u32(tiles);
   const uint32_t fb = (uint32_t)(fieldsz * SZ), sb = 3u * fb;
   long long g_next = ((long long)(i0 - 1) * p.nyh + (jr0 + p.h - 1)) * nz;  // next plane to load
+  const uint64_t l2pol = l2_policy(p.l2hint);
   int to_issue = nsteps + 1, s_next = 0;  // planes i0-1 .. i1
   uint32_t par_next = 0;  // parity of the empty-phase the next refill of slot s_next waits for
   auto issue_plane = [&]() {
     const uint32_t full = bar0 + 8 * s_next;
     mbar_expect_tx(full, 3 * tile_bytes);
     const uint32_t dst = t0 + (uint32_t)s_next * sb;
-    tma_load_1d(dst, u + g_next, tile_bytes, full);
-    tma_load_1d(dst + fb, v + g_next, tile_bytes, full);
-    tma_load_1d(dst + 2 * fb, w + g_next, tile_bytes, full);
+    if (p.l2hint) {
+      tma_load_1d_hint(dst, u + g_next, tile_bytes, full, l2pol);
+      tma_load_1d_hint(dst + fb, v + g_next, tile_bytes, full, l2pol);
+      tma_load_1d_hint(dst + 2 * fb, w + g_next, tile_bytes, full, l2pol);
+    } else {
+      tma_load_1d(dst, u + g_next, tile_bytes, full);
+      tma_load_1d(dst + fb, v + g_next, tile_bytes, full);
+      tma_load_1d(dst + 2 * fb, w + g_next, tile_bytes, full);
+    }
     g_next += p.plane;
     --to_issue;
     if (++s_next == nstages) s_next = 0;
@@ -530,6 +556,15 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
       " [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+      : "memory");
+}
+// the same copy with an L2 eviction-priority hint for the lines it reads
+__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap *map, int c0, int c1,
+                                                 int c2, uint32_t bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4}], [%5], %6;"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
       : "memory");
 }
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *map) {
@@ -814,6 +849,7 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
     pdl_wait();  // the fields may have been written by the previous kernel in the stream
     const uint32_t dst0 = t0 + (uint32_t)(lane * fieldsz * SZ);
     const int G = p.colgroup;
+    const uint64_t l2pol = l2_policy(p.l2hint);
     const int jcfirst = jr0 + p.h - 1;  // array column of the tile's first row
     const uint32_t cbs = (uint32_t)ragged_class_bytes(rows, G);
     int s = 0;
@@ -827,8 +863,12 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
       if constexpr (!RAG) {
         if (lane == 0) mbar_expect_tx(full, (uint32_t)nfld * box_bytes);
         __syncwarp();
-        if (lane < nfld)
-          tma_load_3d(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+        if (lane < nfld) {
+          if (p.l2hint)
+            tma_load_3d_hint(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full, l2pol);
+          else
+            tma_load_3d(dst0 + (uint32_t)(s * stagesz * SZ), mymap, kb0 - NK, jr0 + p.h - 1, i0 - 1 + n, full);
+        }
       } else {
         // ragged nz (a column is not a whole number of 16-byte vectors): the descriptor views G
         // columns as one row (G nz elements: a multiple of 16 bytes), so column j is the elements
@@ -841,8 +881,11 @@ tma_scalars(const KParams<T> p, const __grid_constant__ TensorMaps maps, const S
         for (int idx = lane; idx < nfld * G; idx += 32) {
           const int f = idx / G, c = idx - f * G;
           const int e0 = c * nz;  // the column's first level in its row of the view
-          tma_load_3d(t0 + (uint32_t)((s * stagesz + f * fieldsz) * SZ) + (uint32_t)c * cbs,
-                      &maps.m[f < 3 ? f : s0 + f], e0 - e0 % NK + kb0 - NK, (jcfirst - c + G - 1) / G, i0 - 1 + n, full);
+          const uint32_t dst = t0 + (uint32_t)((s * stagesz + f * fieldsz) * SZ) + (uint32_t)c * cbs;
+          const CUtensorMap *map = &maps.m[f < 3 ? f : s0 + f];
+          const int cz = e0 - e0 % NK + kb0 - NK, cy = (jcfirst - c + G - 1) / G;
+          if (p.l2hint) tma_load_3d_hint(dst, map, cz, cy, i0 - 1 + n, full, l2pol);
+          else tma_load_3d(dst, map, cz, cy, i0 - 1 + n, full);
         }
       }
       if (++s == nstages) { s = 0; par ^= 1; }
