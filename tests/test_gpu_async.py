@@ -229,6 +229,35 @@ def test_config2_and_3_full_size_every_element(cid):
     L.close()
 
 
+def test_ragged_nz_full_size_every_element():
+    # bench.py's `ragged_nz` record: config 2 with one level less (512x512x255 fp64, 3 + 10 fields,
+    # the fused launch on the grouped-column view), every interior element of all 13 outputs
+    cfg = dataclasses.replace(synth.CONFIGS[2], nz=255)
+    P, L = gc.make_pair(cfg)
+    nthr = oracle.max_threads()
+    U, V, W = [synth.field(cfg, n) for n in "uvw"]
+    names = synth.field_names(cfg)
+    d = [gc.to_dev(a, L) for a in (U, V, W)]
+    dq = [gc.to_dev(synth.field(cfg, n), L) for n in names]
+    fo = gc.fresh_out(L, 3 + cfg.nq)
+    L.tendencies(*d, fo[0], fo[1], fo[2], dq, fo[3:])
+    torch.cuda.synchronize()
+    assert "tma_fused" in L.describe_plan() and "colgroup=2" in L.describe_plan(), L.describe_plan()
+    errs = {}
+    want = P.momentum(U, V, W, nthreads=nthr)
+    for idx, nm in enumerate(("su", "sv", "sw")):
+        errs[nm] = gc.check(cfg, fo[idx], want[idx], nm)
+        gc.check_halo_untouched(cfg, fo[idx], nm)
+    del want
+    sq = np.zeros(P.shape)
+    for idx, nm in enumerate(names):
+        P.scalar(U, V, W, synth.field(cfg, nm), nthreads=nthr, out=sq)
+        errs[nm] = gc.check(cfg, fo[3 + idx], sq, nm)
+        gc.check_halo_untouched(cfg, fo[3 + idx], nm)
+    print("ragged nz = 255 full-array max rel errs:", {k: f"{a:.1e}" for k, a in errs.items()})
+    L.close()
+
+
 def test_config4_hybrid_async_full_size():
     """1024x1024x160, 3 momentum + 4 scalars in pinned host memory, 8 chunks, the
     20-step loop of BASELINE.json configs[4]: the seeded fields are perturbed every
