@@ -175,9 +175,9 @@ def config_record(cfg, workload, **extra):
 # kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
 # by (workload, kernel family); valid for the library's default launch plan only.
 NCU_TRAFFIC = {
-    ("config1", "tma_momentum"): (357.2e6, "profiles/r02_config1_tma_momentum.md"),
-    ("config2", "tma_fused"): (14918.3e6, "profiles/r02_config2_tma_fused.md"),
-    ("config3", "tma_fused"): (7126.1e6, "profiles/r02_config3_tma_fused.md"),
+    ("config1", "tma_momentum"): (357.7e6, "profiles/r02_config1_tma_momentum.md"),
+    ("config2", "tma_fused"): (14789.7e6, "profiles/r02_config2_tma_fused.md"),
+    ("config3", "tma_fused"): (7115.6e6, "profiles/r02_config3_tma_fused.md"),
 }
 
 
@@ -417,6 +417,25 @@ def run_device_config(ctx, args, workload, cache, headline):
                tile_y=args.tile_y, warps=args.warps, split=args.split, pdl=not args.no_pdl, form=args.form,
                launch_plan=plan)}
 
+    rec["field_points_per_s_G"] = value * nf  # grid points x advected fields
+    if headline and not swap:
+        # SURVEY.md 8(d) timing protocol: >= 20 launches timed one by one, median and best
+        ctx.barrier()
+        evs = []
+        with torch.cuda.stream(st):
+            for i in range(3):
+                whole_step(i)
+            for i in range(21):
+                e = torch.cuda.Event(enable_timing=True)
+                e.record(st)
+                evs.append(e)
+                if i < 20:
+                    whole_step(i)
+        ctx.barrier()
+        per = sorted(a.elapsed_time(b) for a, b in zip(evs[:-1], evs[1:]))
+        rec["roofline"]["per_launch_ms"] = {"launches": 20, "median": float(np.median(per)), "best": per[0],
+                                            "median_GBs": alg / (float(np.median(per)) * 1e-3) / 1e9,
+                                            "best_GBs": alg / (per[0] * 1e-3) / 1e9}
     # ---- sustained: the same step for >= args.sustain_seconds (the board reaches its power
     # cap within about a second; sw_power_cap is noted, not rejected)
     if args.sustain_seconds > 0 and not swap:
@@ -721,6 +740,85 @@ def run_hybrid_config(ctx, args, steps, warmup, with_cpu):
     return rec
 
 
+def run_paper_shape(ctx, args):
+    """Context: the paper's own per-process sub-domain, 64x64x64 = 262144 points
+    (PAPER.md:105-111), 3 momentum + theta + 5 q, through the hybrid step; alone, and 8 such
+    sub-domains sharing the GPU as the paper's 8 MPI ranks shared a K20X: 8 handles,
+    every step enqueued before any is waited for.  Timing only (seeded host fields)."""
+    torch = ctx.torch
+    from paper_2009_12850_b200 import binding, synth
+    cfg = synth.Config(90, 64, 64, 64, halo=2, nq=6, dtype="f64")
+    g = synth.grid(cfg.nz)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    ranks = []
+    for _ in range(8):
+        L = binding.MoncAdv(cfg.nx, cfg.ny, cfg.nz, cfg.halo, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"],
+                            dtype="f64")
+        hin = [torch.from_numpy(a).pin_memory() for a in H]
+        hout = [torch.zeros(L.shape, dtype=torch.float64).pin_memory() for _ in names]
+        ranks.append((L, hin, hout))
+
+    def enqueue(r):
+        L, hin, hout = r
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+
+    def timed(rs, n):
+        for _ in range(3):
+            for r in rs:
+                enqueue(r)
+            for r in rs:
+                r[0].step_wait()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n):
+            for r in rs:
+                enqueue(r)
+            for r in rs:
+                r[0].step_wait()
+        return (time.perf_counter() - t0) / n
+
+    t1 = timed(ranks[:1], 50)
+    t8 = timed(ranks, 20)
+    pts = cfg.nx * cfg.ny * cfg.nz
+    out = {"config": {"workload": "paper sub-domain 64x64x64, 3 + 6 fields, hybrid step", "nx": 64, "ny": 64, "nz": 64,
+                      "nq": 6, "storage_dtype": "f64", "step_call": "monc_adv_step_async + monc_adv_step_wait"},
+           "one_subdomain": {"ms_per_step": t1 * 1e3, "value": pts / t1 / 1e9, "chunks": ranks[0][0].step_chunk_count()},
+           "eight_subdomains_sharing_the_gpu": {"ms_per_round": t8 * 1e3, "value": 8 * pts / t8 / 1e9,
+                                                "speedup_over_one_after_another": 8 * t1 / t8},
+           "unit": "Gpts/s", "launch_plan": ranks[0][0].describe_plan()}
+    for L, _, _ in ranks:
+        L.close()
+    del ranks
+    gc.collect()
+    # the paper's strong-scaling domain (PAPER.md:107: z = 64, x = y = 2048, 268 M points; 1024 K20X nodes at
+    # the far end of Fig. 4) resident in ONE B200's HBM: the same 3 + 6 fields, one fused launch per step
+    nx = ny = 2048
+    L = binding.MoncAdv(nx, ny, 64, 2, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"], dtype="f64")
+    gen = torch.Generator(device="cuda").manual_seed(20091285)
+    ins = [torch.randn(L.shape, device="cuda", dtype=torch.float64, generator=gen) for _ in range(9)]
+    outs = [torch.empty(L.shape, device="cuda", dtype=torch.float64) for _ in range(9)]
+    st = torch.cuda.Stream()
+
+    def whole(i):
+        L.tendencies(ins[0], ins[1], ins[2], outs[0], outs[1], outs[2], ins[3:], outs[3:], stream=st)
+
+    e0, e1 = timed_loop(ctx, st, whole, 5, warm=2)
+    ctx.barrier()
+    ms = e0.elapsed_time(e1) / 5
+    alg = bytes_fused(6, "f64") * nx * ny * 64
+    peak, _ = peaks()
+    out["global_domain_2048x2048x64_resident"] = {
+        "ms_per_step": ms, "value": nx * ny * 64 / (ms * 1e-3) / 1e9, "algorithmic_GBs": alg / (ms * 1e-3) / 1e9,
+        "frac": alg / (ms * 1e-3) / 1e9 / peak, "hbm_resident_GB": 18 * L.shape[0] * L.shape[1] * L.shape[2] * 8 / 1e9,
+        "launch_plan": L.describe_plan(), "steps": 5, "data": "device randn (timing only)"}
+    L.close()
+    del ins, outs
+    gc.collect()
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ragged_nz(ctx, args):
     """Config 2 with one level less (512x512x255 fp64, 3 + 10 fields): nz is not a whole number of
     16-byte vectors, the shape round 1 sent to the one-thread-per-point kernels.  Timing only (device
@@ -802,10 +900,11 @@ def run_ours(args):
             except Exception as e:  # a sub-record must not take the headline down with it
                 others[w] = {"error": f"{type(e).__name__}: {e}"}
             if w == "config1":
-                try:
-                    others["ragged_nz"] = run_ragged_nz(ctx, args)
-                except Exception as e:
-                    others["ragged_nz"] = {"error": f"{type(e).__name__}: {e}"}
+                for key, fn in (("ragged_nz", run_ragged_nz), ("paper_subdomain", run_paper_shape)):
+                    try:
+                        others[key] = fn(ctx, args)
+                    except Exception as e:
+                        others[key] = {"error": f"{type(e).__name__}: {e}"}
     if ctx.rank != 0:
         ctx.close()
         return
@@ -815,7 +914,7 @@ def run_ours(args):
            "data": "synthetic", "config": rec["config"], "roofline": rec["roofline"],
            "cpu_baseline": rec.get("cpu_baseline"), "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
            "clocks": rec["clocks"]}
-    for k in ("sustained", "burst", "two_call_step", "work_scale_16"):
+    for k in ("field_points_per_s_G", "sustained", "burst", "two_call_step", "work_scale_16"):
         if k in rec:
             out[k] = rec[k]
     if others:

@@ -312,7 +312,15 @@ cudaError_t launch_pdl(monc_adv_t h, void (*kernel)(KArgs...), dim3 grid, int cl
     attr[1].val.clusterDim.z = 1;
     cfg.numAttrs = 2;
   }
-  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+  cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+  if (e != cudaSuccess && cluster > 1 && e != cudaErrorInvalidResourceHandle) {
+    // clusters are a placement hint only (no kernel uses distributed shared memory): if this
+    // device or partition cannot co-schedule them, launch the same grid without
+    cudaGetLastError();
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+  }
+  return e;
 }
 
 template <typename T>
@@ -698,11 +706,20 @@ template <typename T>
 int launch_tendencies(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *sv, T *sw,
                       const void *const *q, void *const *sq, int nq, int ia, int ib, cudaStream_t st) {
   if (nq > 0 && h->fuse && (h->variant == 3 || h->variant == 0)) {
+    // the fused launch takes one scalar group (10 scalars); further scalars follow in a scalars
+    // launch of their own, which re-reads the wind (24 of 24 + 16 n bytes per point)
     KParams<T> p = make_params<T>(h, ia, ib);
     const MomPtrs<T> mo{su, sv, sw};
+    const int nfused = std::min(nq, 10);
     bool done = false;
-    const int rc = run_tma_scalars<T>(h, p, u, v, w, q, sq, nq, ia, ib, st, &done, &mo);
-    if (rc != MONC_ADV_OK || done) return rc;
+    const int rc = run_tma_scalars<T>(h, p, u, v, w, q, sq, nfused, ia, ib, st, &done, &mo);
+    if (rc != MONC_ADV_OK || (done && nfused == nq)) return rc;
+    if (done) {
+      const std::string fused_plan = h->plan_sca;
+      const int rc2 = launch_scalars<T>(h, u, v, w, q + nfused, sq + nfused, nq - nfused, ia, ib, st);
+      h->plan_mom = fused_plan;
+      return rc2;
+    }
   }
   const int rc = launch_momentum<T>(h, u, v, w, su, sv, sw, ia, ib, st);
   if (rc != MONC_ADV_OK || nq == 0) return rc;

@@ -415,6 +415,38 @@ def test_ragged_nz_on_the_tma_kernels(shape):
         L.close()
 
 
+@pytest.mark.parametrize("cluster", [2, 3, 4, 8])
+def test_cluster_launches_are_a_placement_hint_only(cluster):
+    # thread-block clusters of y-neighbour tiles (monc_adv_set_cluster): the grid is padded to whole
+    # clusters, the extra blocks exit; results bitwise those of the plain launch
+    for nz, tuning in ((200, dict(tile_y=2, xchunk=5)), (200, dict()), (129, dict(tile_y=3, xchunk=4))):
+        cfg = gc.custom_cfg(11, 18, nz, nq=4, cid=740)  # ny + 2 halo even: the ragged nz = 129 takes the TMA kernels too
+        P, L = gc.make_pair(cfg)
+        L.set_tuning(**tuning)
+        names = ["u", "v", "w"] + synth.field_names(cfg)
+        D = [gc.to_dev(synth.field(cfg, n), L) for n in names]
+        res = []
+        for cl in (1, cluster):
+            L.set_cluster(cl)
+            o = gc.fresh_out(L, 7)
+            L.momentum(D[0], D[1], D[2], *o[:3])
+            # (the size is capped at the y-tile count; the text after ";" is the last scalars launch)
+            assert ("cluster=1 " in L.describe_plan().split(";")[0]) == (cl == 1), L.describe_plan()
+            L.scalars(D[3:], o[3:])
+            o2 = gc.fresh_out(L, 7)
+            L.tendencies(D[0], D[1], D[2], o2[0], o2[1], o2[2], D[3:], o2[3:])
+            assert ("cluster=1 " in L.describe_plan()) == (cl == 1), L.describe_plan()
+            torch.cuda.synchronize()
+            res.append(o + o2)
+        for a, b in zip(*res):
+            assert torch.equal(a, b)
+        want = P.momentum(*[synth.field(cfg, n) for n in "uvw"])
+        for o, w_, n in zip(res[1][:3], want, ("su", "sv", "sw")):
+            gc.check(cfg, o, w_, n)
+            gc.check_halo_untouched(cfg, o, n)
+        L.close()
+
+
 @pytest.mark.parametrize("dtype,nz", [("f64", 1100), ("f32", 2200), ("f64", 1101)])
 def test_tall_columns_take_the_tensor_map_kernel(dtype, nz):
     # more than 16 warps per column: tma_momentum (whole columns per block) does not fit, the z-tiled
@@ -550,10 +582,12 @@ def test_tendencies_fused(dtype, form):
                        (7, dict(xchunk=8, warps=2)), (10, dict(xchunk=6))):
         plan = run_tendencies(cfg, nq, form=form, tuning=tuning)
         assert "tma_fused" in plan, plan
-    # nothing to fuse / too many scalars for one group: two launches, same results
+    # nothing to fuse: the momentum launch alone; fusing switched off: two launches, same results
     assert "tma_fused" not in run_tendencies(cfg, 0, form=form)
-    assert "tma_fused" not in run_tendencies(cfg, 11, form=form)
     assert "tma_fused" not in run_tendencies(cfg, 4, form=form, fuse=False)
+    # more scalars than the fused launch's one group of 10: the rest in a scalars launch of their own
+    plan = run_tendencies(cfg, 13, form=form)
+    assert "tma_fused(momentum+scalars) group=10" in plan and "; tma_scalars group=3" in plan, plan
 
 
 def test_tendencies_accumulate_and_shapes():
