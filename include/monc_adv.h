@@ -189,6 +189,11 @@ int monc_adv_step_times_ms(monc_adv_t h, float out[4]);
  * the library choose per step from the bytes on the host link and the fixed cost
  * of a chunk (a step takes T (1 + 1/C) + C c). */
 int monc_adv_set_chunks(monc_adv_t h, int nchunks);
+/* The chunk count an automatic step would take for this shape, nfields_in arrays up and
+ * nfields_out arrays down (3 + nq each for a full step; twice nfields_out up with
+ * accumulate): the power of two nearest to sqrt(T / c).  Needs no handle and no GPU.
+ * Returns the count (>= 1) or MONC_ADV_EINVAL. */
+int monc_adv_plan_chunks(int nx, int ny, int nz, int halo, int dtype, int nfields_in, int nfields_out);
 /* Chunk count of the step in flight (or of the last one); with a fixed count, that
  * count.  0 = automatic and no step enqueued yet. */
 int monc_adv_step_chunk_count(monc_adv_t h);

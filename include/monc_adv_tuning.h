@@ -46,6 +46,15 @@ int monc_adv_set_cluster(monc_adv_t h, int n);
  * steps later --, 0 no hint, 2 evict_first (for measurements). */
 int monc_adv_set_l2_hint(monc_adv_t h, int hint);
 
+/* The launch geometry the planners choose for a full-domain call on this shape, as text
+ * (the format of monc_adv_describe_plan), for a device with sm_count SMs and smem_optin
+ * bytes of opt-in shared memory per block (B200: 148, 232448).  fused != 0: the plan of
+ * monc_adv_tendencies (the first 10 scalars); else monc_adv_momentum and, if nq > 0,
+ * monc_adv_scalars.  Host arithmetic only: needs no handle and no GPU (the planners'
+ * regression tests run on it).  buf receives at most buflen - 1 characters. */
+int monc_adv_plan_describe(int nx, int ny, int nz, int halo, int dtype, int nq, int fused, int sm_count,
+                           int smem_optin, char *buf, int buflen);
+
 /* 1 (default): the TMA kernels are launched with CUDA's programmatic
  * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
  * predecessor in the stream (it waits for the predecessor's completion before

@@ -28,13 +28,33 @@ MAX_SCALARS = 64
 SYMBOLS = [
     "monc_adv_create", "monc_adv_destroy", "monc_adv_momentum", "monc_adv_bind_wind",
     "monc_adv_scalars", "monc_adv_tendencies", "monc_adv_set_fuse", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
-    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range", "monc_adv_step_chunk_count",
+    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range", "monc_adv_step_chunk_count", "monc_adv_plan_chunks", "monc_adv_plan_describe",
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
     "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version", "monc_adv_set_work_scale",
     "monc_adv_set_cluster", "monc_adv_set_l2_hint",
 ]
+
+
+def plan_chunks(nx, ny, nz, halo, dtype, nfields_in, nfields_out) -> int:
+    """The chunk count an automatic hybrid step would take (no handle, no GPU)."""
+    dt = {"f64": F64, "f32": F32}.get(dtype, dtype)
+    n = load().monc_adv_plan_chunks(int(nx), int(ny), int(nz), int(halo), int(dt), int(nfields_in), int(nfields_out))
+    if n < 1:
+        raise MoncAdvError(n, "plan_chunks: bad argument")
+    return n
+
+
+def plan_describe(nx, ny, nz, halo, dtype, nq, fused=True, sm_count=148, smem_optin=232448) -> str:
+    """The launch geometry the library's planners choose for this shape (no handle, no GPU)."""
+    dt = {"f64": F64, "f32": F32}.get(dtype, dtype)
+    buf = C.create_string_buffer(640)
+    rc = load().monc_adv_plan_describe(int(nx), int(ny), int(nz), int(halo), int(dt), int(nq), int(bool(fused)),
+                                       int(sm_count), int(smem_optin), buf, len(buf))
+    if rc != OK:
+        raise MoncAdvError(rc, "plan_describe: bad argument")
+    return buf.value.decode()
 
 
 class MoncAdvError(RuntimeError):
@@ -90,6 +110,10 @@ def load():
     lib.monc_adv_step_wait_chunk.restype = ci
     lib.monc_adv_step_chunk_range.argtypes = [vp, ci, C.POINTER(ci), C.POINTER(ci)]
     lib.monc_adv_step_chunk_range.restype = ci
+    lib.monc_adv_plan_describe.argtypes = [ci] * 9 + [C.c_char_p, ci]
+    lib.monc_adv_plan_describe.restype = ci
+    lib.monc_adv_plan_chunks.argtypes = [ci] * 7
+    lib.monc_adv_plan_chunks.restype = ci
     lib.monc_adv_step_chunk_count.argtypes = [vp]
     lib.monc_adv_step_chunk_count.restype = ci
     lib.monc_adv_step_times_ms.argtypes = [vp, C.POINTER(C.c_float)]

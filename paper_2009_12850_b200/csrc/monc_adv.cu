@@ -38,6 +38,7 @@ struct TmaPlan {
   bool ok = false;
   int ty = 0, stages = 0, xc = 0, tiles = 0, nchunks = 0;
   int cl = 1;  // thread-block cluster: cl y-neighbour tiles are co-scheduled on one GPC
+  bool cl_checked = false;  // the default cluster size has been checked against the device's resident clusters
   size_t smem = 0;
 };
 // geometry of tma_scalars: ty columns x ss scalar splits = consumer warps per
@@ -65,6 +66,7 @@ struct monc_adv_s {
   // is a whole number of 16-byte vectors whatever nz is (1 when nz already is; 2 or 4 when nz is
   // ragged; 0 = no such view: nyh is not a multiple of it, the generic kernels run)
   int colgroup = 1;
+  bool plan_only = false;  // a shape without a device behind it (monc_adv_plan_describe)
   double dx = 0, dy = 0;
   size_t elems = 0, esize = 8;
   int device = 0;
@@ -341,6 +343,33 @@ int launch_momentum(monc_adv_t h, const T *u, const T *v, const T *w, T *su, T *
     dim3 grid((pl.tiles + pl.cl - 1) / pl.cl * pl.cl, pl.nchunks);  // padded to whole clusters: the extra blocks exit
     auto go = [&](auto kernel) -> int {
       CU(allow_max_smem(h, kernel));
+      if (pl.cl > 1 && h->cluster == 0 && !pl.cl_checked) {
+        // the default clusters are worth it only if every cluster of the (padded) grid is resident at
+        // once: a GPC of 18 SMs holds 4 clusters of 4, and clusters left over run as a second wave
+        // (config 1 with 37 y tiles: 3460 GB/s in clusters of 4 against 5650 without)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid;
+        cfg.blockDim = dim3((unsigned)(pl.ty * p.wzc * 32));
+        cfg.dynamicSmemBytes = pl.smem;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)pl.cl;
+        attr[0].val.clusterDim.y = attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        int resident = 0;
+        if (cudaOccupancyMaxActiveClusters(&resident, kernel, &cfg) != cudaSuccess) {
+          cudaGetLastError();
+          resident = 0;
+        }
+        if ((long)grid.x / pl.cl * grid.y > resident) {
+          pl.cl = 1;
+          grid.x = (unsigned)pl.tiles;
+        }
+        TmaPlan &kept = h->mom_plans[ib - ia];  // remembered: the query runs once per plan
+        kept.cl = pl.cl;
+        kept.cl_checked = true;
+      }
       CU(launch_pdl(h, kernel, grid, pl.cl, pl.ty * p.wzc * 32, pl.smem, st, p, pl.ty, pl.stages, u, v, w, su, sv, sw));
       return MONC_ADV_OK;
     };
@@ -428,7 +457,7 @@ template <typename T>
 TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mom) {
   TmaScalarPlan pl;
   constexpr int NK = VecOf<T>::NK;
-  if (h->colgroup == 0 || !tensor_map_encoder()) return pl;
+  if (h->colgroup == 0 || (!h->plan_only && !tensor_map_encoder())) return pl;
   if (n == 0 && !mom) return pl;
   const size_t budget = (size_t)std::min(h->smem_optin, 227 * 1024) - 1024;
   const int nch_fixed = h->xchunk > 0 ? (nplanes + h->xchunk - 1) / h->xchunk : 0;
@@ -747,8 +776,8 @@ void free_staging(monc_adv_t h) {
 // events, a kernel launch).  Minimum at C = sqrt(T / c).  Measured on B200 / PCIe Gen5 x16
 // (DESIGN.md 7.3): both directions at once move 49.5 GB/s each, c = 15 us + 5 us per copy
 // (config 4: 212 ms at C = 8, 201 ms at 32..64; config 2: 158 ms at 8, 151 ms at 32; config 1's shape: 8).
-int auto_chunks(monc_adv_t h, int nf_in, int nf_out) {
-  const double bytes = (double)std::max(nf_in, nf_out) * (double)h->nx * h->nyh * h->nz * (double)h->esize;
+int auto_chunks_for(int nx, int nyh, int nz, size_t esize, int nf_in, int nf_out) {
+  const double bytes = (double)std::max(nf_in, nf_out) * (double)nx * nyh * nz * (double)esize;
   const double t_ms = bytes / 49.5e6;
   const double c_ms = 0.015 + 0.005 * (nf_in + nf_out);
   // the power of two nearest to sqrt(T / c): equal slabs copy measurably better than ragged
@@ -756,8 +785,11 @@ int auto_chunks(monc_adv_t h, int nf_in, int nf_out) {
   const double want = std::sqrt(t_ms / c_ms);
   int c = 1;
   while (c < 64 && (double)(2 * c) * (2 * c) <= want * want * 2.0) c *= 2;  // 2c <= want * sqrt(2)
-  while (c > h->nx) c /= 2;
+  while (c > nx) c /= 2;
   return std::max(1, c);
+}
+int auto_chunks(monc_adv_t h, int nf_in, int nf_out) {
+  return auto_chunks_for(h->nx, h->nyh, h->nz, h->esize, nf_in, nf_out);
 }
 int step_chunks(monc_adv_t h, int nf_in, int nf_out) {
   return h->nchunks > 0 ? std::min(h->nchunks, h->nx) : auto_chunks(h, nf_in, nf_out);
@@ -1192,6 +1224,64 @@ int monc_adv_step_wait(monc_adv_t h) {
   h->times[3] = t;
   h->have_times = true;
   return MONC_ADV_OK;
+}
+
+int monc_adv_plan_describe(int nx, int ny, int nz, int halo, int dtype, int nq, int fused, int sm_count,
+                           int smem_optin, char *buf, int buflen) {
+  if (nx < 1 || ny < 1 || nz < 3 || halo < 1 || nq < 0 || nq > 20 || !buf || buflen < 1 || sm_count < 1 ||
+      smem_optin < 1024 || (dtype != MONC_ADV_F64 && dtype != MONC_ADV_F32))
+    return MONC_ADV_EINVAL;
+  monc_adv_s hs;  // a shape only: no CUDA call is made through it
+  monc_adv_t h = &hs;
+  h->plan_only = true;
+  h->nx = nx; h->ny = ny; h->nz = nz; h->h = halo; h->dtype = dtype;
+  h->nxh = nx + 2 * halo; h->nyh = ny + 2 * halo;
+  h->esize = dtype == MONC_ADV_F64 ? 8 : 4;
+  h->sm_count = sm_count; h->smem_optin = smem_optin;
+  int g = 1;
+  while (((size_t)g * nz * h->esize) % 16 != 0) g *= 2;
+  h->colgroup = h->nyh % g == 0 ? g : 0;
+  char b[320];
+  const bool f64 = dtype == MONC_ADV_F64;
+  std::string text;
+  if (!fused || nq == 0) {
+    const TmaPlan pm = f64 ? compute_plan_tma<double>(h, nx, 3) : compute_plan_tma<float>(h, nx, 3);
+    if (pm.ok) {
+      snprintf(b, sizeof b, "tma_momentum ty=%d stages=%d xc=%d grid=%dx%d cluster=%d smem=%zu", pm.ty, pm.stages,
+               pm.xc, (pm.tiles + pm.cl - 1) / pm.cl * pm.cl, pm.nchunks, pm.cl, pm.smem);
+      text = b;
+    } else {
+      const TmaScalarPlan pr = f64 ? compute_plan_tma_scalars<double>(h, nx, 0, true)
+                                   : compute_plan_tma_scalars<float>(h, nx, 0, true);
+      if (pr.ok) {
+        snprintf(b, sizeof b, "tma_fused(momentum role only) ty=%d stages=%d xc=%d grid=%dx%d colgroup=%d smem=%zu",
+                 pr.ty, pr.stages, pr.xc, pr.tiles, pr.nchunks, h->colgroup, pr.smem);
+        text = b;
+      } else {
+        text = "no TMA plan (momentum)";
+      }
+    }
+  }
+  if (nq > 0) {
+    const TmaScalarPlan ps = f64 ? compute_plan_tma_scalars<double>(h, nx, std::min(nq, fused ? 10 : nq), fused != 0)
+                                 : compute_plan_tma_scalars<float>(h, nx, std::min(nq, fused ? 10 : nq), fused != 0);
+    if (ps.ok)
+      snprintf(b, sizeof b, "%s group=%d per_warp=%d split=%d ty=%d stages=%d xc=%d grid=%dx%d cluster=%d colgroup=%d smem=%zu",
+               fused ? "tma_fused(momentum+scalars)" : "tma_scalars", ps.gb, ps.gw, ps.ss, ps.ty, ps.stages, ps.xc,
+               ps.tiles, ps.nchunks, ps.cl, std::max(1, h->colgroup), ps.smem);
+    else
+      snprintf(b, sizeof b, "no TMA plan (scalars)");
+    text += (text.empty() ? "" : "; ") + std::string(b);
+  }
+  snprintf(buf, (size_t)buflen, "%s", text.c_str());
+  return MONC_ADV_OK;
+}
+
+int monc_adv_plan_chunks(int nx, int ny, int nz, int halo, int dtype, int nfields_in, int nfields_out) {
+  if (nx < 1 || ny < 1 || nz < 1 || halo < 1 || nfields_in < 1 || nfields_out < 1 ||
+      (dtype != MONC_ADV_F64 && dtype != MONC_ADV_F32))
+    return MONC_ADV_EINVAL;
+  return auto_chunks_for(nx, ny + 2 * halo, nz, dtype == MONC_ADV_F64 ? 8 : 4, nfields_in, nfields_out);
 }
 
 int monc_adv_step_chunk_count(monc_adv_t h) {

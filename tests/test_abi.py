@@ -37,7 +37,7 @@ def test_header_symbols_all_exported(lib):
     assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of sync with the headers"
     # the kernel-geometry knobs live in the internal header only
     public = declared_functions((HEADER,))
-    for n in ("monc_adv_set_tuning", "monc_adv_set_variant", "monc_adv_set_pdl", "monc_adv_set_cluster", "monc_adv_set_l2_hint"):
+    for n in ("monc_adv_set_tuning", "monc_adv_set_variant", "monc_adv_set_pdl", "monc_adv_set_cluster", "monc_adv_set_l2_hint", "monc_adv_plan_describe"):
         assert n not in public and n in names
 
 
@@ -96,3 +96,18 @@ def test_product_does_not_import_oracle():
     otxt = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + \
         open(os.path.join(ROOT, "oracle", "monc_adv_oracle.cpp")).read()
     assert "paper_2009_12850_b200" not in otxt.replace("paper_2009_12850_b200/csrc", "")
+
+
+def test_plan_chunks_host_rule(lib):
+    # a hybrid step takes T (1 + 1/C) + C c; the library takes the power of two nearest
+    # sqrt(T / c) with T = bytes of one direction at 49.5 GB/s, c = 15 us + 5 us per copy.  Host arithmetic only.
+    assert binding.plan_chunks(512, 512, 256, 2, "f64", 13, 13) == 32    # config 2: measured best 32
+    assert binding.plan_chunks(1024, 1024, 160, 2, "f64", 7, 7) == 64    # config 4: 32..64 measured equal
+    assert binding.plan_chunks(256, 256, 128, 2, "f64", 3, 3) == 8       # config 1's shape: measured best 8
+    assert binding.plan_chunks(512, 512, 256, 2, "f32", 13, 13) == 16    # half the bytes
+    assert binding.plan_chunks(16, 16, 32, 2, "f64", 3, 3) == 1          # config 0: one chunk
+    assert binding.plan_chunks(3, 2048, 256, 2, "f64", 13, 13) <= 3      # never more chunks than x planes
+    counts = [binding.plan_chunks(n, n, 128, 2, "f64", 5, 5) for n in (32, 64, 128, 256, 512, 1024, 2048)]
+    assert counts == sorted(counts) and all(c & (c - 1) == 0 for c in counts) and counts[-1] <= 64
+    with pytest.raises(binding.MoncAdvError):
+        binding.plan_chunks(0, 4, 4, 2, "f64", 3, 3)
