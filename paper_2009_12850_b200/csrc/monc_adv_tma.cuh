@@ -45,7 +45,29 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Wait for the phase with parity `parity` of an mbarrier, called by ALL 32 lanes of a converged
+// warp.  The lanes leave the spin loop TOGETHER (vote.sync.all on the try_wait results): the
+// result of try_wait is per lane, and lanes that left a plain spin loop at different
+// iterations stay diverged afterwards -- the compiler sees straight-line inline asm, assumes
+// convergence and turns the __syncwarp() before a slot release into a NOP, so that lane 0's
+// group could release a ring slot while the other group had not yet issued its last shared-
+// memory read of it (seen as one launch in ~50 at config 2 reading a plane's u four planes late:
+// DESIGN.md 11).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1, P2;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, 2000;\n"  // suspend for up to 2 us per attempt
+      "vote.sync.all.pred P2, P1, 0xffffffff;\n"
+      "@P2 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(bar), "r"(parity)
+      : "memory");
+}
+// the same wait for a single lane (tma_momentum's refilling lane, inside a divergent branch)
+__device__ __forceinline__ void mbar_wait_one(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred P1;\n"
@@ -519,7 +541,7 @@ tma_momentum(const KParams<T> p, const int ty, const int nstages, const T *__res
   momentum_march<T, ACC, SKEW, WS, false>(m, [&]() {
     if (producer && to_issue > 0) {
       // slot of plane i-1: every warp released it during the previous step
-      mbar_wait(bar0 + 8 * (nstages + s_next), par_next);
+      mbar_wait_one(bar0 + 8 * (nstages + s_next), par_next);
       chk_jitter(3);
       chk_poison(t0 + (uint32_t)s_next * sb, sb, 0, 1);
       issue_plane();

@@ -1,0 +1,81 @@
+"""Repeat-and-compare stress runs of the ring kernels at config 2's size.
+
+The kernels are deterministic (no atomics, fixed summation order), so every launch on the same inputs must give
+the same bits.  A ring-protocol fault that depends on timing (a slot read after it was refilled, or before it was
+full) shows up as a launch that differs from the first -- which is how the fault fixed in round 2 was found: lanes
+that left the mbarrier spin loop at different iterations stayed diverged, lane 0's group released a slot while the
+other group had not yet issued its last read of it, and about one fused config-2 launch in 50 used, for one warp and
+one x face, the u of the plane four planes further on.  One comparison with the oracle per launch
+would take minutes; bitwise equality with a launch that test_gpu_async.py checks against the oracle takes seconds."""
+import pytest
+import torch
+
+from paper_2009_12850_b200 import binding, synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _need_gpu(gpu_required):
+    yield
+    torch.cuda.synchronize()
+
+
+def repeat_and_compare(nx, ny, nz, nq, dtype, launches, call="tendencies", tuning=None):
+    g = synth.grid(nz)
+    L = binding.MoncAdv(nx, ny, nz, 2, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"], dtype=dtype)
+    if tuning:
+        L.set_tuning(**tuning)
+    tdt = L.torch_dtype
+    gen = torch.Generator(device="cuda").manual_seed(12850)
+    a = [torch.randn(L.shape, device="cuda", dtype=tdt, generator=gen) for _ in range(3 + nq)]
+    ref = [torch.full(L.shape, -777.25, device="cuda", dtype=tdt) for _ in range(3 + nq)]
+    out = [torch.full(L.shape, -777.25, device="cuda", dtype=tdt) for _ in range(3 + nq)]
+
+    def run(o):
+        if call == "tendencies":
+            L.tendencies(a[0], a[1], a[2], o[0], o[1], o[2], a[3:], o[3:])
+        else:
+            L.momentum(a[0], a[1], a[2], o[0], o[1], o[2])
+            if nq:
+                L.scalars(a[3:], o[3:])
+
+    run(ref)
+    torch.cuda.synchronize()
+    plan = L.describe_plan()
+    bad = []
+    for rep in range(launches):
+        run(out)
+        for f, (x, y) in enumerate(zip(ref, out)):
+            if not torch.equal(x, y):
+                d = (x != y).nonzero()
+                bad.append((rep, f, d.shape[0], d[0].tolist(), d[-1].tolist()))
+    L.close()
+    assert not bad, f"{len(bad)} (launch, field) pairs differ from the first launch, e.g. {bad[:4]}; plan: {plan}"
+    return plan
+
+
+def test_fused_step_repeats_bitwise_fp64():
+    # config 2's size; 150 launches: the round-2 fault showed in ~2 % of these launches
+    assert "tma_fused" in repeat_and_compare(512, 512, 256, 10, "f64", 150)
+
+
+def test_fused_step_repeats_bitwise_fp32():
+    assert "tma_fused" in repeat_and_compare(512, 512, 256, 10, "f32", 150)
+
+
+def test_two_calls_repeat_bitwise():
+    plan = repeat_and_compare(512, 512, 256, 10, "f64", 60, call="two")
+    assert "tma_momentum" in plan and "tma_scalars" in plan
+
+
+def test_short_rings_and_small_tiles_repeat_bitwise():
+    # the shallowest rings and the smallest tiles: the producer is closest behind the consumers
+    repeat_and_compare(256, 256, 128, 4, "f64", 60, tuning=dict(stages=3, tile_y=2, xchunk=16))
+    repeat_and_compare(256, 256, 128, 7, "f64", 60, call="two", tuning=dict(stages=2, tile_y=2, split=3, xchunk=16))
+    repeat_and_compare(256, 256, 128, 0, "f64", 200, call="two")  # config 1's momentum launch
+
+
+def test_ragged_nz_repeats_bitwise():
+    assert "colgroup=2" in repeat_and_compare(512, 512, 255, 10, "f64", 60)
+    assert "momentum role only" in repeat_and_compare(256, 256, 127, 0, "f64", 100, call="two")
