@@ -55,6 +55,17 @@ int monc_adv_set_l2_hint(monc_adv_t h, int hint);
 int monc_adv_plan_describe(int nx, int ny, int nz, int halo, int dtype, int nq, int fused, int sm_count,
                            int smem_optin, char *buf, int buflen);
 
+/* 1 (default): a hybrid step whose arguments and settings equal those of the step before it
+ * is captured into a CUDA graph and replayed from then on (one cudaGraphLaunch instead of the
+ * ~30 CUDA calls of every chunk).  0: every step is enqueued call by call.  Results and the
+ * completion calls (step_inputs_consumed / step_wait_chunk / step_wait / step_times_ms) are the
+ * same either way. */
+int monc_adv_set_graph(monc_adv_t h, int on);
+/* 0: graphs are off (set_graph(0), or a capture failed on this driver and the handle fell back
+ * to call-by-call enqueues); 1: on, no step captured at the moment; 2: the last step was a
+ * captured step (the next one with the same arguments is a replay). */
+int monc_adv_graph_state(monc_adv_t h);
+
 /* 1 (default): the TMA kernels are launched with CUDA's programmatic
  * stream-serialisation attribute, so a kernel's set-up overlaps the tail of its
  * predecessor in the stream (it waits for the predecessor's completion before

@@ -33,7 +33,7 @@ SYMBOLS = [
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
     "monc_adv_describe_plan", "monc_adv_last_error", "monc_adv_version", "monc_adv_set_work_scale",
-    "monc_adv_set_cluster", "monc_adv_set_l2_hint",
+    "monc_adv_set_cluster", "monc_adv_set_l2_hint", "monc_adv_set_graph", "monc_adv_graph_state",
 ]
 
 
@@ -110,6 +110,8 @@ def load():
     lib.monc_adv_step_wait_chunk.restype = ci
     lib.monc_adv_step_chunk_range.argtypes = [vp, ci, C.POINTER(ci), C.POINTER(ci)]
     lib.monc_adv_step_chunk_range.restype = ci
+    lib.monc_adv_graph_state.argtypes = [vp]
+    lib.monc_adv_graph_state.restype = ci
     lib.monc_adv_plan_describe.argtypes = [ci] * 9 + [C.c_char_p, ci]
     lib.monc_adv_plan_describe.restype = ci
     lib.monc_adv_plan_chunks.argtypes = [ci] * 7
@@ -120,7 +122,8 @@ def load():
     lib.monc_adv_step_times_ms.restype = ci
     for name in ("monc_adv_set_chunks", "monc_adv_set_overlap", "monc_adv_set_form",
                  "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
-                 "monc_adv_set_fuse", "monc_adv_set_work_scale", "monc_adv_set_cluster", "monc_adv_set_l2_hint"):
+                 "monc_adv_set_fuse", "monc_adv_set_work_scale", "monc_adv_set_cluster", "monc_adv_set_l2_hint",
+                 "monc_adv_set_graph"):
         getattr(lib, name).argtypes = [vp, ci]
         getattr(lib, name).restype = ci
     lib.monc_adv_set_tuning.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci]
@@ -296,6 +299,12 @@ class MoncAdv:
 
     def set_pdl(self, on):
         self._check(self._lib.monc_adv_set_pdl(self._h, int(bool(on))))
+
+    def graph_state(self) -> int:
+        return int(self._lib.monc_adv_graph_state(self._h))
+
+    def set_graph(self, on):
+        self._check(self._lib.monc_adv_set_graph(self._h, int(bool(on))))
 
     def set_l2_hint(self, hint):
         self._check(self._lib.monc_adv_set_l2_hint(self._h, int(hint)))

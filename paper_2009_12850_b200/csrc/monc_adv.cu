@@ -95,7 +95,16 @@ struct monc_adv_s {
   std::vector<void *> d_in, d_out;  // 3+nq each
   cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
   cudaEvent_t ev_user = nullptr, ev_in_begin = nullptr, ev_out_begin = nullptr;
-  std::vector<cudaEvent_t> ev_h2d, ev_kb, ev_ke, ev_d2h;
+  std::vector<cudaEvent_t> ev_h2d, ev_kb, ev_ke, ev_d2h;  // what the host waits on / times (per chunk)
+  std::vector<cudaEvent_t> dep_h2d, dep_ke;               // cross-stream dependencies inside a step (per chunk)
+  cudaEvent_t dep_join_k = nullptr, dep_join_out = nullptr, ev_done = nullptr;
+  // the enqueue of a step with unchanged arguments is captured once into a CUDA graph and replayed
+  int use_graph = 1;
+  unsigned long epoch = 0;             // bumped by every setter: a graph never outlives a setting
+  std::vector<uintptr_t> graph_key;    // arguments + settings of the captured step
+  std::vector<uintptr_t> pending_key;  // of the last step that was enqueued eagerly
+  cudaGraphExec_t graph_exec = nullptr;
+  long graph_launches = 0;             // kernels one replay launches
   std::vector<int> chunk_a, chunk_b;  // interior-relative x ranges of the in-flight step
   bool in_flight = false, have_times = false;
   float times[4] = {0, 0, 0, 0};
@@ -803,6 +812,9 @@ int ensure_async_objects(monc_adv_t h, int nq, int nchunks) {
     CU(cudaEventCreateWithFlags(&h->ev_user, cudaEventDisableTiming));
     CU(cudaEventCreate(&h->ev_in_begin));
     CU(cudaEventCreate(&h->ev_out_begin));
+    CU(cudaEventCreateWithFlags(&h->dep_join_k, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&h->dep_join_out, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming));
   }
   while ((int)h->ev_h2d.size() < nchunks) {
     cudaEvent_t a, b, c, d;
@@ -810,6 +822,9 @@ int ensure_async_objects(monc_adv_t h, int nq, int nchunks) {
     CU(cudaEventCreate(&c)); CU(cudaEventCreate(&d));
     h->ev_h2d.push_back(a); h->ev_kb.push_back(b);
     h->ev_ke.push_back(c); h->ev_d2h.push_back(d);
+    CU(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    h->dep_h2d.push_back(a); h->dep_ke.push_back(b);
   }
   if (h->staged_nq < nq) {
     // grow: keep what exists, add the missing scalar buffers
@@ -851,7 +866,13 @@ void drain_internal_streams(monc_adv_t h) {
 template <typename T>
 int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw,
                     const void *const *hq, int nq, void *hsu, void *hsv, void *hsw,
-                    void *const *hsq, cudaStream_t user) {
+                    void *const *hsq, bool capture) {
+  // capture = the calls below are being captured into a CUDA graph (s_in is the origin
+  // stream): events the host waits on or times are then recorded as external event nodes
+  // (they fire at every replay), the cross-stream dependencies as ordinary captured events
+  auto host_event = [&](cudaEvent_t ev, cudaStream_t st) {
+    return capture ? cudaEventRecordWithFlags(ev, st, cudaEventRecordExternal) : cudaEventRecord(ev, st);
+  };
   const bool mom = hsu != nullptr;
   const int C = step_chunks(h, 3 + nq, ((mom ? 3 : 0) + nq) * (h->accumulate ? 2 : 1));
   const size_t es = sizeof(T);
@@ -867,10 +888,6 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
   cudaStream_t sk = h->overlap ? h->s_k : h->s_in;
   cudaStream_t sout = h->overlap ? h->s_out : h->s_in;
 
-  if (user) {
-    CU(cudaEventRecord(h->ev_user, user));
-    CU(cudaStreamWaitEvent(sin, h->ev_user, 0));
-  }
   h->chunk_a.assign(C, 0);
   h->chunk_b.assign(C, 0);
   for (int c = 0; c < C; ++c) {
@@ -882,7 +899,7 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
   std::vector<void *> dsq(std::max(nq, 1));
   for (int n = 0; n < nq; ++n) { dq[n] = h->d_in[3 + n]; dsq[n] = h->d_out[3 + n]; }
 
-  CU(cudaEventRecord(h->ev_in_begin, sin));
+  CU(host_event(h->ev_in_begin, sin));
   // ---- H2D: planes [h-1, h+nx] split so that chunk c's kernels need chunks <= c only
   auto h2d_chunk = [&](int c) -> int {
     const int lo = (c == 0) ? h->h - 1 : h->h + h->chunk_b[c - 1] + 1;
@@ -900,13 +917,14 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
         CU(cudaMemcpy2DAsync((char *)h->d_out[n] + ooff, plane_b, hout[n] + ooff, plane_b, width,
                              (size_t)(ib - ia), cudaMemcpyHostToDevice, sin));
     }
-    CU(cudaEventRecord(h->ev_h2d[c], sin));
+    CU(host_event(h->ev_h2d[c], sin));
+    CU(cudaEventRecord(h->dep_h2d[c], sin));
     return MONC_ADV_OK;
   };
   auto compute_chunk = [&](int c) -> int {
     const int ia = h->h + h->chunk_a[c], ib = h->h + h->chunk_b[c];
-    if (h->overlap) CU(cudaStreamWaitEvent(sk, h->ev_h2d[c], 0));
-    CU(cudaEventRecord(h->ev_kb[c], sk));
+    if (h->overlap) CU(cudaStreamWaitEvent(sk, h->dep_h2d[c], 0));
+    CU(host_event(h->ev_kb[c], sk));
     int rc = MONC_ADV_OK;
     if (mom)
       rc = launch_tendencies<T>(h, du, dv, dw, (T *)h->d_out[0], (T *)h->d_out[1], (T *)h->d_out[2],
@@ -914,20 +932,21 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
     else if (nq > 0)
       rc = launch_scalars<T>(h, du, dv, dw, dq.data(), dsq.data(), nq, ia, ib, sk);
     if (rc != MONC_ADV_OK) return rc;
-    CU(cudaEventRecord(h->ev_ke[c], sk));
+    CU(host_event(h->ev_ke[c], sk));
+    CU(cudaEventRecord(h->dep_ke[c], sk));
     return MONC_ADV_OK;
   };
   auto d2h_chunk = [&](int c) -> int {
     const int ia = h->h + h->chunk_a[c], ib = h->h + h->chunk_b[c];
-    if (h->overlap) CU(cudaStreamWaitEvent(sout, h->ev_ke[c], 0));
-    if (c == 0) CU(cudaEventRecord(h->ev_out_begin, sout));
+    if (h->overlap) CU(cudaStreamWaitEvent(sout, h->dep_ke[c], 0));
+    if (c == 0) CU(host_event(h->ev_out_begin, sout));
     // interior columns only: 2-D copy, one row per x plane
     const size_t off = ((size_t)ia * h->nyh + h->h) * h->nz * es;
     const size_t width = (size_t)h->ny * h->nz * es;
     for (int n = mom ? 0 : 3; n < nf; ++n)
       CU(cudaMemcpy2DAsync(hout[n] + off, plane_b, (char *)h->d_out[n] + off, plane_b, width,
                            (size_t)(ib - ia), cudaMemcpyDeviceToHost, sout));
-    CU(cudaEventRecord(h->ev_d2h[c], sout));
+    CU(host_event(h->ev_d2h[c], sout));
     return MONC_ADV_OK;
   };
   int rc;
@@ -942,7 +961,81 @@ int step_async_impl(monc_adv_t h, const void *hu, const void *hv, const void *hw
     for (int c = 0; c < C; ++c) if ((rc = compute_chunk(c)) != MONC_ADV_OK) return rc;
     for (int c = 0; c < C; ++c) if ((rc = d2h_chunk(c)) != MONC_ADV_OK) return rc;
   }
-  if (user) CU(cudaStreamWaitEvent(user, h->ev_d2h[C - 1], 0));
+  if (h->overlap) {
+    // the kernel and D2H streams rejoin s_in: s_in is complete when the step is (and a
+    // capture needs every forked stream joined before it ends)
+    CU(cudaEventRecord(h->dep_join_k, sk));
+    CU(cudaEventRecord(h->dep_join_out, sout));
+    CU(cudaStreamWaitEvent(sin, h->dep_join_k, 0));
+    CU(cudaStreamWaitEvent(sin, h->dep_join_out, 0));
+  }
+  return MONC_ADV_OK;
+}
+
+void drop_graph(monc_adv_t h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  h->graph_exec = nullptr;
+  h->graph_key.clear();
+}
+
+// Enqueue one hybrid step.  A step whose arguments and settings equal those of the step before
+// it is captured into a CUDA graph (all three streams, every copy, launch and event) and from
+// then on replayed with ONE cudaGraphLaunch: the enqueue of config 2's 32-chunk step costs the
+// host 1.5-1.9 ms call by call (about 900 CUDA calls), a replay a few tens of microseconds
+// (DESIGN.md 8).  The first step with new arguments is enqueued call by call (it also fills
+// the plan and descriptor caches, so that a capture makes stream calls only).
+template <typename T>
+int step_async_enqueue(monc_adv_t h, const void *hu, const void *hv, const void *hw, const void *const *hq, int nq,
+                       void *hsu, void *hsv, void *hsw, void *const *hsq, cudaStream_t user) {
+  std::vector<uintptr_t> key = {(uintptr_t)hu, (uintptr_t)hv, (uintptr_t)hw, (uintptr_t)hsu, (uintptr_t)hsv,
+                                (uintptr_t)hsw, (uintptr_t)nq, (uintptr_t)h->epoch};
+  for (int n = 0; n < nq; ++n) { key.push_back((uintptr_t)hq[n]); key.push_back((uintptr_t)hsq[n]); }
+  cudaStream_t sin = h->s_in;
+  if (user) {
+    CU(cudaEventRecord(h->ev_user, user));
+    CU(cudaStreamWaitEvent(sin, h->ev_user, 0));
+  }
+  const bool graphs = h->use_graph && h->overlap;
+  int rc = MONC_ADV_OK;
+  if (graphs && h->graph_exec && key == h->graph_key) {
+    CU(cudaGraphLaunch(h->graph_exec, sin));  // chunk ranges, plans: those of the captured step
+    h->launches += h->graph_launches;
+  } else if (graphs && key == h->pending_key) {
+    drop_graph(h);
+    const long l0 = h->launches;
+    cudaGraph_t graph = nullptr;
+    CU(cudaStreamBeginCapture(sin, cudaStreamCaptureModeThreadLocal));
+    rc = step_async_impl<T>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, true);
+    const cudaError_t ec = cudaStreamEndCapture(sin, &graph);  // (ends an invalidated capture too)
+    const std::string why = h->err;
+    if (rc == MONC_ADV_OK && ec == cudaSuccess && graph &&
+        cudaGraphInstantiate(&h->graph_exec, graph, 0) == cudaSuccess) {
+      h->graph_launches = h->launches - l0;
+      h->graph_key = key;
+      cudaGraphDestroy(graph);
+      CU(cudaGraphLaunch(h->graph_exec, sin));
+    } else {
+      // a capture that does not work on this driver is not an error of the step: enqueue it call
+      // by call, and do not try again on this handle
+      if (graph) cudaGraphDestroy(graph);
+      cudaGetLastError();
+      h->graph_exec = nullptr;
+      h->use_graph = 0;
+      h->launches = l0;
+      h->err = why;
+      rc = step_async_impl<T>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, false);
+      if (rc != MONC_ADV_OK) return rc;
+    }
+  } else {
+    if (graphs && h->graph_exec) drop_graph(h);
+    rc = step_async_impl<T>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, false);
+    if (rc != MONC_ADV_OK) return rc;
+    h->pending_key = key;
+  }
+  if (user) {
+    CU(cudaEventRecord(h->ev_done, sin));
+    CU(cudaStreamWaitEvent(user, h->ev_done, 0));
+  }
   h->in_flight = true;
   h->have_times = false;
   return MONC_ADV_OK;
@@ -1046,6 +1139,11 @@ void monc_adv_destroy(monc_adv_t h) {
   for (void *p : h->d_tz) if (p) cudaFree(p);
   for (auto v : {&h->ev_h2d, &h->ev_kb, &h->ev_ke, &h->ev_d2h})
     for (cudaEvent_t ev : *v) cudaEventDestroy(ev);
+  drop_graph(h);
+  for (auto v : {&h->dep_h2d, &h->dep_ke})
+    for (cudaEvent_t ev : *v) cudaEventDestroy(ev);
+  for (cudaEvent_t ev : {h->dep_join_k, h->dep_join_out, h->ev_done})
+    if (ev) cudaEventDestroy(ev);
   if (h->ev_user) cudaEventDestroy(h->ev_user);
   if (h->ev_in_begin) cudaEventDestroy(h->ev_in_begin);
   if (h->ev_out_begin) cudaEventDestroy(h->ev_out_begin);
@@ -1140,6 +1238,7 @@ int monc_adv_tendencies(monc_adv_t h, const void *u, const void *v, const void *
 
 int monc_adv_set_fuse(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   h->fuse = on ? 1 : 0;
   return MONC_ADV_OK;
 }
@@ -1172,8 +1271,8 @@ int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void
   rc = ensure_async_objects(h, nq, step_chunks(h, 3 + nq, ((hsu ? 3 : 0) + nq) * (h->accumulate ? 2 : 1)));
   if (rc) return rc;
   cudaStream_t user = (cudaStream_t)cuda_stream;
-  rc = h->dtype == MONC_ADV_F64 ? step_async_impl<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user)
-                                : step_async_impl<float>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
+  rc = h->dtype == MONC_ADV_F64 ? step_async_enqueue<double>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user)
+                                : step_async_enqueue<float>(h, hu, hv, hw, hq, nq, hsu, hsv, hsw, hsq, user);
   if (rc != MONC_ADV_OK) {
     // part of the step may already be queued: let it finish (it touches only the caller's
     // arrays of this call and the staging buffers), then report; the handle stays usable
@@ -1309,6 +1408,7 @@ int monc_adv_step_times_ms(monc_adv_t h, float out[4]) {
 
 int monc_adv_set_chunks(monc_adv_t h, int nchunks) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_chunks: step in flight");
   if (nchunks < 0 || nchunks > h->nx) return fail(h, MONC_ADV_EINVAL, "set_chunks: need 0 (automatic) or 1 <= nchunks <= nx");
   h->nchunks = nchunks;
@@ -1319,6 +1419,7 @@ int monc_adv_set_chunks(monc_adv_t h, int nchunks) {
 
 int monc_adv_set_overlap(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_overlap: step in flight");
   h->overlap = on ? 1 : 0;
   return MONC_ADV_OK;
@@ -1326,6 +1427,7 @@ int monc_adv_set_overlap(monc_adv_t h, int on) {
 
 int monc_adv_set_form(monc_adv_t h, int form) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (form != MONC_ADV_FORM_FLUX && form != MONC_ADV_FORM_PW_SKEW)
     return fail(h, MONC_ADV_EINVAL, "set_form: unknown form");
   if (form != MONC_ADV_FORM_FLUX && h->work > 1) return fail(h, MONC_ADV_EINVAL, "set_form: work scaling is on (flux form only)");
@@ -1335,6 +1437,7 @@ int monc_adv_set_form(monc_adv_t h, int form) {
 
 int monc_adv_set_accumulate(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (on && h->work > 1) return fail(h, MONC_ADV_EINVAL, "set_accumulate: work scaling is on (overwrite mode only)");
   if ((on ? 1 : 0) != h->accumulate) h->mom_plans.clear();  // the accumulating momentum kernel takes fewer warps
   h->accumulate = on ? 1 : 0;
@@ -1343,6 +1446,7 @@ int monc_adv_set_accumulate(monc_adv_t h, int on) {
 
 int monc_adv_set_work_scale(monc_adv_t h, int n) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (n < 1 || n > 64) return fail(h, MONC_ADV_EINVAL, "set_work_scale: need 1 <= n <= 64");
   if (n > 1 && (h->form != MONC_ADV_FORM_FLUX || h->accumulate || (h->variant != 0 && h->variant != 3)))
     return fail(h, MONC_ADV_EINVAL, "set_work_scale: needs the flux form, overwrite mode and the TMA kernels");
@@ -1353,6 +1457,7 @@ int monc_adv_set_work_scale(monc_adv_t h, int n) {
 
 int monc_adv_set_cluster(monc_adv_t h, int n) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (n < 0 || n > 8) return fail(h, MONC_ADV_EINVAL, "set_cluster: 0 (default) or 1..8");
   h->cluster = n;
   h->mom_plans.clear();
@@ -1362,19 +1467,35 @@ int monc_adv_set_cluster(monc_adv_t h, int n) {
 
 int monc_adv_set_l2_hint(monc_adv_t h, int hint) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (hint < 0 || hint > 2) return fail(h, MONC_ADV_EINVAL, "set_l2_hint: 0 (none), 1 (evict_last) or 2 (evict_first)");
   h->l2hint = hint;
   return MONC_ADV_OK;
 }
 
+int monc_adv_set_graph(monc_adv_t h, int on) {
+  if (!h) return MONC_ADV_EINVAL;
+  if (h->in_flight) return fail(h, MONC_ADV_EBUSY, "set_graph: step in flight");
+  h->epoch++;
+  h->use_graph = on ? 1 : 0;
+  return MONC_ADV_OK;
+}
+
+int monc_adv_graph_state(monc_adv_t h) {
+  if (!h || !h->use_graph) return 0;
+  return h->graph_exec ? 2 : 1;
+}
+
 int monc_adv_set_pdl(monc_adv_t h, int on) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   h->pdl = on ? 1 : 0;
   return MONC_ADV_OK;
 }
 
 int monc_adv_set_variant(monc_adv_t h, int variant) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;  // a captured step never outlives a setting
   if (variant < 0 || variant > 3) return fail(h, MONC_ADV_EINVAL, "set_variant: 0..3");
   if (h->work > 1 && variant != 0 && variant != 3)
     return fail(h, MONC_ADV_EINVAL, "set_variant: work scaling is on (TMA kernels only)");
@@ -1391,6 +1512,7 @@ int monc_adv_set_variant(monc_adv_t h, int variant) {
 int monc_adv_set_tuning(monc_adv_t h, int xchunk, int group, int prefetch, int warps, int stages,
                         int tile_y, int split) {
   if (!h) return MONC_ADV_EINVAL;
+  h->epoch++;
   if (xchunk < 0 || group < 0 || group > 10 || prefetch < -1 || prefetch > 16 || warps < 0 ||
       warps > kWarpsPerBlock || stages < 0 || stages > 8 || tile_y < 0 || split < 0 || split > 4)
     return fail(h, MONC_ADV_EINVAL, "set_tuning: value out of range");

@@ -37,7 +37,7 @@ def test_header_symbols_all_exported(lib):
     assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of sync with the headers"
     # the kernel-geometry knobs live in the internal header only
     public = declared_functions((HEADER,))
-    for n in ("monc_adv_set_tuning", "monc_adv_set_variant", "monc_adv_set_pdl", "monc_adv_set_cluster", "monc_adv_set_l2_hint", "monc_adv_plan_describe"):
+    for n in ("monc_adv_set_tuning", "monc_adv_set_variant", "monc_adv_set_pdl", "monc_adv_set_cluster", "monc_adv_set_l2_hint", "monc_adv_plan_describe", "monc_adv_set_graph", "monc_adv_graph_state"):
         assert n not in public and n in names
 
 

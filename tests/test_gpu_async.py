@@ -148,6 +148,70 @@ def test_step_async_ragged_nz(nz, dtype):
     L.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("accumulate", [False, True])
+def test_step_async_graph_replay(dtype, accumulate):
+    # a step whose arguments equal those of the step before is captured into a CUDA graph and replayed:
+    # step 1 call by call, step 2 captured + launched, steps 3.. replayed.  The host changes its fields
+    # between steps (same arrays); every step must equal the call-by-call enqueue bitwise, the per-chunk
+    # completion calls and the timing record must keep working, a setter must drop the graph
+    cfg = gc.custom_cfg(24, 12, 64, nq=3, dtype=dtype, cid=407)
+    P, L = gc.make_pair(cfg)
+    _, Lref = gc.make_pair(cfg)
+    Lref.set_graph(False)
+    for lib in (L, Lref):
+        lib.set_chunks(4)
+        lib.set_accumulate(accumulate)
+    names = ["u", "v", "w"] + synth.field_names(cfg)
+    H = [synth.field(cfg, n) for n in names]
+    hin = [pinned(a, L) for a in H]
+    hout, href = pinned_out(L, 6), pinned_out(L, 6)
+    h = cfg.halo
+    rng = np.random.default_rng(5)
+    for step in range(1, 7):
+        if step == 5:
+            L.set_form("flux")   # any setter drops the graph: this step is enqueued call by call again
+        for t in hin:                # the model moves on: new values in the same pinned arrays
+            t.numpy()[...] += rng.normal(0.0, 0.01, size=t.shape).astype(t.numpy().dtype)
+        if accumulate:               # in/out source terms: both start from the same host values
+            for a_, b_ in zip(hout, href):
+                a_.numpy()[h:h + cfg.nx, h:h + cfg.ny] = step
+                b_.numpy()[h:h + cfg.nx, h:h + cfg.ny] = step
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+        assert L.step_chunk_count() == 4
+        # steps 1 and 5 (new settings) go call by call, 2 and 6 are captured, 3 and 4 replayed
+        assert L.graph_state() == (1 if step in (1, 5) else 2), (step, L.graph_state())
+        assert Lref.graph_state() == 0
+        L.step_inputs_consumed()
+        covered = 0
+        for c in range(4):           # streaming combine on a replayed step
+            L.step_wait_chunk(c)
+            a, b = L.step_chunk_range(c)
+            covered += b - a
+        assert covered == cfg.nx
+        L.step_wait()
+        t = L.step_times_ms()
+        assert t["total"] > 0 and t["kernels"] > 0 and t["h2d"] > 0 and t["d2h"] > 0
+        Lref.step_async(hin[0], hin[1], hin[2], hin[3:], href[0], href[1], href[2], href[3:])
+        Lref.step_wait()
+        for a_, b_, n in zip(hout, href, ["su", "sv", "sw"] + names[3:]):
+            assert torch.equal(a_, b_), (step, n)
+        if not accumulate:
+            U, V, W = (t_.numpy().astype(np.float64) for t_ in hin[:3])
+            for o, w_, n in zip(hout[:3], P.momentum(U, V, W), ("su", "sv", "sw")):
+                gc.check(cfg, o, w_, f"{n}[step {step}]")
+    # 6 steps x 4 chunks, one fused launch each, replayed launches counted too
+    assert L.launch_count() == 24 and Lref.launch_count() == 24
+    # a user stream: the step starts after the stream's work and the stream waits for the step
+    st = torch.cuda.Stream()
+    for _ in range(3):
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:], stream=st)
+        st.synchronize()
+        L.step_wait()
+    L.close()
+    Lref.close()
+
+
 def test_step_async_pw_skew():
     # the hybrid step in the PW-skew form (NEXT-1): x-slab launches of the TMA kernels
     cfg = gc.custom_cfg(24, 17, 128, nq=4, cid=403)
