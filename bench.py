@@ -175,9 +175,9 @@ def config_record(cfg, workload, **extra):
 # kernel, from the committed `--set full` captures under profiles/ (bytes).  Keyed
 # by (workload, kernel family); valid for the library's default launch plan only.
 NCU_TRAFFIC = {
-    ("config1", "tma_momentum"): (357.7e6, "profiles/r02_config1_tma_momentum.md"),
-    ("config2", "tma_fused"): (14789.7e6, "profiles/r02_config2_tma_fused.md"),
-    ("config3", "tma_fused"): (7115.6e6, "profiles/r02_config3_tma_fused.md"),
+    ("config1", "tma_momentum"): (356.8e6, "profiles/r02_config1_tma_momentum.md"),
+    ("config2", "tma_fused"): (14600.6e6, "profiles/r02_config2_tma_fused.md"),
+    ("config3", "tma_fused"): (7109.4e6, "profiles/r02_config3_tma_fused.md"),
 }
 
 
