@@ -243,6 +243,13 @@ __device__ __forceinline__ Vec<T> lds_row(uint32_t a, const T *tag) {
   if constexpr (RAG) return lds_elems(a, tag);
   else return lds_at<0>(a, tag);
 }
+// a neighbour row at a compile-time byte offset OFF (aligned columns: the offset folds into the
+// instruction) or, RAG, at the warp's run-time offset `rs` (row stride +- the shift between the rows)
+template <bool RAG, int OFF, typename T>
+__device__ __forceinline__ Vec<T> lds_nb(uint32_t a, uint32_t rs, const T *tag) {
+  if constexpr (RAG) return lds_elems(OFF < 0 ? a - rs : a + rs, tag);
+  else return lds_at<OFF>(a, tag);
+}
 // coefficient vector of levels k0 .. k0+NK-1; RAG: element by element, 0 outside the column
 template <bool RAG, typename T>
 __device__ __forceinline__ Vec<T> ld_coef(const T *tz, const int k0, const int nz) {
@@ -691,7 +698,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
     mbar_wait(bar0 + 8 * st, par);  // the next plane has landed
     chk_jitter(4);
     const uint32_t pV = pA + fb, pW = pV + fb;
-    Vec<T> vs = lds_row<RAG>(pV - rsbS, tag), vn = lds_at<0>(pV, tag);
+    Vec<T> vs = lds_nb<RAG, -kRowBytes>(pV, rsbS, tag), vn = lds_at<0>(pV, tag);
     Vec<T> wt = lds_at<0>(pW, tag);
     Vec<T> wl = down_with(wt, lds1_at<-SZ>(pW, tag));  // w one level below each element
     un = lds_at<0>(pA, tag);  // read now: the slot's release must not wait for it
@@ -707,7 +714,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
       if (FULL || s < mycnt) {  // warp-uniform
         QN[s] = lds_at<0>(pQ, tag);
         const Vec<T> &q = QN[s];
-        const Vec<T> qS = lds_row<RAG>(pQ - rsbS, tag), qN = lds_row<RAG>(pQ + rsbN, tag);
+        const Vec<T> qS = lds_nb<RAG, -kRowBytes>(pQ, rsbS, tag), qN = lds_nb<RAG, kRowBytes>(pQ, rsbN, tag);
         const T qtop = lds1_at<UP>(pQ, tag);  // the level above the thread's last
         // the level below the thread's first: lane 0 reads it, the others get it by shuffle
         const T qb = bot_edge ? lds1_at<-SZ>(pQ, tag) : T(0);
