@@ -45,6 +45,9 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+#ifndef MONC_ADV_WAIT_HINT
+#define MONC_ADV_WAIT_HINT 1  // try_wait with a suspend-time hint (measured against the plain form: DESIGN.md 7.2)
+#endif
 // Wait for the phase with parity `parity` of an mbarrier, called by ALL 32 lanes of a converged
 // warp.  The lanes leave the spin loop TOGETHER (vote.sync.all on the try_wait results): the
 // result of try_wait is per lane, and lanes that left a plain spin loop at different
@@ -58,7 +61,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "{\n"
       ".reg .pred P1, P2;\n"
       "LAB_WAIT:\n"
+#if MONC_ADV_WAIT_HINT
       "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, 2000;\n"  // suspend for up to 2 us per attempt
+#else
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+#endif
       "vote.sync.all.pred P2, P1, 0xffffffff;\n"
       "@P2 bra DONE;\n"
       "bra LAB_WAIT;\n"
@@ -135,6 +142,7 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 #ifndef MONC_ADV_CHECKED
 #define MONC_ADV_CHECKED 0
 #endif
+
 __device__ __forceinline__ void chk_jitter(const unsigned salt) {
 #if MONC_ADV_CHECKED
   unsigned x = (unsigned)clock64() * 2654435761u + salt * 40503u + blockIdx.x * 9176u + (threadIdx.x >> 5) * 7919u;
