@@ -79,3 +79,30 @@ def test_short_rings_and_small_tiles_repeat_bitwise():
 def test_ragged_nz_repeats_bitwise():
     assert "colgroup=2" in repeat_and_compare(512, 512, 255, 10, "f64", 60)
     assert "momentum role only" in repeat_and_compare(256, 256, 127, 0, "f64", 100, call="two")
+
+
+def test_hybrid_step_repeats_bitwise():
+    # the hybrid step on one set of pinned arrays, 40 times: call by call, captured, then replayed from the
+    # CUDA graph; every step must land the bits of the first in host memory (chunked launches of the fused
+    # kernel, three streams, copies in both directions at once)
+    nx, ny, nz, nq = 256, 256, 128, 4
+    g = synth.grid(nz)
+    L = binding.MoncAdv(nx, ny, nz, 2, synth.DX, synth.DY, g["dz"], g["dzn"], g["rho"], g["rhon"], dtype="f64")
+    gen = torch.Generator().manual_seed(12851)
+    hin = [torch.randn(L.shape, dtype=torch.float64, generator=gen).pin_memory() for _ in range(3 + nq)]
+    hout = [torch.full(L.shape, -777.25, dtype=torch.float64).pin_memory() for _ in range(3 + nq)]
+    ref = None
+    bad = []
+    for rep in range(40):
+        for o in hout:
+            o.fill_(-777.25)
+        L.step_async(hin[0], hin[1], hin[2], hin[3:], hout[0], hout[1], hout[2], hout[3:])
+        L.step_wait()
+        if ref is None:
+            ref = [o.clone() for o in hout]
+            assert all(bool((r[2:2 + nx, 2:2 + ny] != -777.25).any()) for r in ref)
+        else:
+            bad += [(rep, f) for f, (x, y) in enumerate(zip(ref, hout)) if not torch.equal(x, y)]
+    assert L.graph_state() == 2
+    L.close()
+    assert not bad, bad[:6]
