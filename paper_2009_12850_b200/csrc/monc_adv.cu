@@ -242,11 +242,19 @@ TmaPlan compute_plan_tma(monc_adv_t h, int nplanes, int fields_per_stage) {
   for (int ty = ty_hi; ty >= ty_lo; --ty) {
     const size_t stage = (size_t)fields_per_stage * (ty + 2) * h->nz * sizeof(T);
     int S = (int)std::min<size_t>(8, budget / (stage + 16));
+    // accumulate: every step waits for the old tendencies of its plane (a read-modify-write the ring
+    // cannot stage); what hides that latency is many short blocks over several waves and a ring that
+    // does not run far ahead of the L2 prefetch of those lines (config 1: 5980 GB/s of real traffic at
+    // 4 stages and 16 planes per block against 2690 with the overwriting launch's geometry)
+    const bool acc = h->accumulate != 0;
+    if (acc) S = std::min(S, 4);
     if (h->stages > 0) S = std::min(S, h->stages);
     if (S < 3) continue;
     const int tiles = (h->ny + ty - 1) / ty;
-    const int nch_lo = nch_fixed ? nch_fixed : 1;
-    const int nch_hi = nch_fixed ? nch_fixed : std::max(1, nplanes / 4);
+    // at least four waves of blocks, of at least 8 planes each
+    const int nch_acc = std::max(1, std::min((4 * h->sm_count + tiles - 1) / tiles, nplanes / 8));
+    const int nch_lo = nch_fixed ? nch_fixed : (acc ? nch_acc : 1);
+    const int nch_hi = nch_fixed ? nch_fixed : std::max(nch_lo, nplanes / 4);
     for (int nch = nch_lo; nch <= nch_hi; ++nch) {
       const int xc = (nplanes + nch - 1) / nch;
       const long blocks = (long)tiles * ((nplanes + xc - 1) / xc);

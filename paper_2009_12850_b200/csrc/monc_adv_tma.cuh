@@ -211,6 +211,12 @@ __device__ __forceinline__ Vec<T> down_with(const Vec<T> &a, const T bot) {
   r.v[0] = bot;
   return r;
 }
+// accumulate mode: the old tendencies of the plane two steps ahead are pulled into L2 now, so
+// that the read-modify-write of that step finds them there (a DRAM miss on every step's critical
+// path made the accumulating launches 2-3.5 x slower than the overwriting ones)
+__device__ __forceinline__ void prefetch_l2(const void *p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 // Element-wise global access for the threads whose 16-byte vector is not whole or not
 // aligned in the caller's array (nz not a multiple of the vector: DESIGN.md 6.8)
 template <typename T>
@@ -344,10 +350,16 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
   // one x step: centre plane in RC (registers) / stage sC, east plane arriving in stage sE.
   // The first step (plane i0-1 as the centre) only builds the x-face terms: no store.
   bool first = true;
+  int left = m.nsteps;  // steps left, the running one included
   auto step = [&](const PlaneRegs<T> &RC, PlaneRegs<T> &RE, const XFlux<T> &FW, XFlux<T> &FE) {
     // accumulate: what the tendencies are added to is read from global memory; issue those
     // loads first so that their latency overlaps the wait for the plane and the arithmetic
     Vec<T> au, av, aw;
+    if (ACC && m.act && left >= 3) {  // this step updates plane c (nothing, the first step), two steps on: c + 2 planes (c + 1)
+      const long long ahead = c + (first ? 1 : 2) * m.plane;
+      prefetch_l2(m.su + ahead); prefetch_l2(m.sv + ahead); prefetch_l2(m.sw + ahead);
+      if (first) { prefetch_l2(m.su + c); prefetch_l2(m.sv + c); prefetch_l2(m.sw + c); }
+    }
     if (ACC) {
 #pragma unroll
       for (int e = 0; e < NK; ++e) au.v[e] = av.v[e] = aw.v[e] = T(0);
@@ -438,7 +450,6 @@ __device__ __forceinline__ void momentum_march(const MarchArgs<T> &m, AfterRelea
     pE += sbytes;
     if (++sE == nstages) { sE = 0; parE ^= 1; pE = a0; }
   };
-  int left = m.nsteps;
 #pragma unroll 1
   while (true) {
     step(RA, RB, FA, FB);
@@ -700,9 +711,18 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
   int st = 0;
   uint32_t par = 0, pA = a0;
   long long c = c0;
+  int togo = nplanes;  // steps left, this one included
 
   auto step = [&](auto store_tag, const Vec<T> (&QP)[GW], Vec<T> (&QN)[GW], const Vec<T> &ux, Vec<T> &un) {
     constexpr bool STORE = decltype(store_tag)::value;
+    if (ACC && act && togo >= 3) {
+      // a storing step updates plane c and pulls plane c + 2 in; the two steps before the first
+      // store (c = c0 in both) pull in the planes the first two stores update
+      const long long ahead = STORE ? c + 2 * plane : c + (nplanes - togo) * plane;
+#pragma unroll
+      for (int s = 0; s < GW; ++s)
+        if (FULL || s < mycnt) prefetch_l2(sqp[s] + ahead);
+    }
     mbar_wait(bar0 + 8 * st, par);  // the next plane has landed
     chk_jitter(4);
     const uint32_t pV = pA + fb, pW = pV + fb;
@@ -805,6 +825,7 @@ __device__ __forceinline__ void scalar_march(const uint32_t a0, const uint32_t f
     __syncwarp();
     if (lane == 0) mbar_arrive(bar0 + 8 * (nstages + st));
     if (STORE) c += plane;
+    --togo;
     pA += sbytes;
     if (++st == nstages) { st = 0; par ^= 1; pA = a0; }
   };
