@@ -474,6 +474,21 @@ def run_device_config(ctx, args, workload, cache, headline):
                                 "value": ctx.world * cfg.points / (wms * 1e-3) / 1e9,
                                 "note": "kernel time with 16 x the arithmetic per byte; the hybrid step through the "
                                         "host link is timed at x16 in other_configs.config4 (PAPER.md:109)"}
+    # ---- accumulate mode (source terms are additive): the same step with
+    # every output a read-modify-write
+    if headline and not swap and not is_tuned(args):
+        ctx.barrier()
+        time.sleep(1.0)
+        L.set_accumulate(True)
+        a0, a1 = timed_loop(ctx, st, whole_step, 10, warm=2)
+        ctx.barrier()
+        L.set_accumulate(False)
+        ams = ctx.max_over_ranks(a0.elapsed_time(a1)) / 10
+        out_b = (3 + nq) * es * cfg.points
+        rec["accumulate"] = {"steps": 10, "ms_per_step": ams, "ratio_to_overwrite": ams / ms_per_step,
+                             "value": ctx.world * cfg.points / (ams * 1e-3) / 1e9,
+                             "bytes_moved_per_step": alg + out_b, "moved_GBs": (alg + out_b) / (ams * 1e-3) / 1e9,
+                             "launch_plan": L.describe_plan()}
     if not headline:
         if cfg.dtype == "f32" and nq:
             # the precision variant end to end (half the bytes on the host link)
@@ -914,7 +929,7 @@ def run_ours(args):
            "data": "synthetic", "config": rec["config"], "roofline": rec["roofline"],
            "cpu_baseline": rec.get("cpu_baseline"), "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
            "clocks": rec["clocks"]}
-    for k in ("field_points_per_s_G", "sustained", "burst", "two_call_step", "work_scale_16"):
+    for k in ("field_points_per_s_G", "sustained", "burst", "two_call_step", "work_scale_16", "accumulate"):
         if k in rec:
             out[k] = rec[k]
     if others:
