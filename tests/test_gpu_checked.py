@@ -79,6 +79,13 @@ def test_checked_ragged_nz():
             tp.test_ragged_nz_on_the_tma_kernels(shape)
 
 
+def test_checked_random_shapes():
+    # the first 60 of the seeded random cases (every launch path) on poisoned, jittered rings
+    import test_gpu_random_shapes as tr
+    for case in tr.CASES[:60]:
+        tr.test_random_shape(case)
+
+
 def test_checked_hybrid_step():
     import test_gpu_async as ta
     for _ in range(REPS):
