@@ -500,13 +500,16 @@ TmaScalarPlan compute_plan_tma_scalars(monc_adv_t h, int nplanes, int n, bool mo
         // one 32-vector z chunk per block tile: the row stride is a compile-time constant
         const int ZB = 32 * NK;
         const int nzt = scalar_z_tiles(h->nz, NK, h->colgroup, h->nz % NK != 0);
-        const int tymax = std::min(h->ny, kScalarConsumerWarps / (ss + (mom ? 1 : 0)));
+        // the momentum role alone (gb = 0) is a chain of dependent steps per warp: two blocks of 7
+        // columns and a 4-stage ring per SM hide its latency better than one block of 15 columns and
+        // a deep ring (256^2 x 127 fp64: 4350 against 3790 GB/s)
+        const int tymax = std::min(h->ny, gb == 0 ? 7 : kScalarConsumerWarps / (ss + (mom ? 1 : 0)));
         if (tymax < 1) continue;
         for (int ty = tymax; ty >= 1; --ty) {
           if (h->tile_y > 0 && ty != std::min(h->tile_y, tymax)) continue;
           const size_t field = (size_t)scalar_field_bytes(ty + 2, h->colgroup, h->nz % NK != 0);
           const size_t stage = (size_t)(3 + gb) * field;
-          int S = (int)std::min<size_t>(8, budget / (stage + 16));
+          int S = (int)std::min<size_t>(gb == 0 ? 4 : 8, budget / (stage + 16));
           if (h->stages > 0) S = std::min(S, h->stages);
           if (S < (mom ? 3 : 2)) continue;
           const int tiles = ((h->ny + ty - 1) / ty) * nzt * ngroups;
