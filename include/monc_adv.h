@@ -185,6 +185,28 @@ int monc_adv_step_chunk_range(monc_adv_t h, int c, int *x_begin, int *x_end);
  * last D2H end, out[3] = whole step (first copy to last copy). */
 int monc_adv_step_times_ms(monc_adv_t h, float out[4]);
 
+/* The momentum step from pinned host memory for callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it): this call
+ * allocates NOTHING on the device -- no cudaMalloc / cudaFree, no stream or event creation,
+ * no allocating library routine.  Its device staging (u, v, w in; su, sv, sw out) is a
+ * file-scope device array of MONC_ADV_NOALLOC_MAX_BYTES that every GPU which loads the
+ * library holds until exit.  Enqueued on `cuda_stream` (NULL = the default stream) and
+ * asynchronous to the host: H2D of the three whole input arrays, the fused su/sv/sw kernel
+ * (the kernel monc_adv_momentum launches), D2H of the interior of the three
+ * tendencies; the host arrays are the caller's until the stream has drained (synchronise
+ * the stream or an event recorded after the call).  Output halos are not written.
+ * Limits: six staged fields must fit, 6 * round_up(NXH * NYH * nz * sizeof(dtype), 256)
+ * <= MONC_ADV_NOALLOC_MAX_BYTES (the paper's 64 x 64 x 64 sub-domain with halo 2 in fp64
+ * fits; BASELINE's configs 1-4 do not: MONC_ADV_EINVAL, nothing enqueued); momentum
+ * only; overwrite mode only; host arrays page-locked and not overlapping.
+ * The scratch is ONE array per device, shared by every handle and every call, and keeps
+ * the last call's contents: nothing in it needs clearing (a call overwrites all it reads
+ * before its kernel runs), but two calls that overlap on the GPU -- different streams, or
+ * different host threads -- race on it.  Calls on one stream are safe back to back. */
+#define MONC_ADV_NOALLOC_MAX_BYTES (16u << 20)
+int monc_adv_step_noalloc(monc_adv_t h, const void *hu, const void *hv, const void *hw, void *hsu, void *hsv,
+                          void *hsw, void *cuda_stream);
+
 /* Number of x-slab chunks of step_async: 1 <= n <= nx, or 0 (the default) to let
  * the library choose per step from the bytes on the host link and the fixed cost
  * of a chunk (a step takes T (1 + 1/C) + C c). */

@@ -23,12 +23,13 @@ F64, F32 = 0, 1
 FORM_FLUX, FORM_PW_SKEW = 0, 1
 OK, EINVAL, ECUDA, ENOMEM, ENOWIND, EBUSY = 0, -1, -2, -3, -4, -5
 MAX_SCALARS = 64
+NOALLOC_MAX_BYTES = 16 << 20  # MONC_ADV_NOALLOC_MAX_BYTES
 
 # every symbol include/monc_adv.h declares (tests check the .so exports them all)
 SYMBOLS = [
     "monc_adv_create", "monc_adv_destroy", "monc_adv_momentum", "monc_adv_bind_wind",
     "monc_adv_scalars", "monc_adv_tendencies", "monc_adv_set_fuse", "monc_adv_step_async", "monc_adv_step_inputs_consumed",
-    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range", "monc_adv_step_chunk_count", "monc_adv_plan_chunks", "monc_adv_plan_describe",
+    "monc_adv_step_wait_chunk", "monc_adv_step_wait", "monc_adv_step_chunk_range", "monc_adv_step_chunk_count", "monc_adv_step_noalloc", "monc_adv_plan_chunks", "monc_adv_plan_describe",
     "monc_adv_step_times_ms", "monc_adv_set_chunks", "monc_adv_set_overlap",
     "monc_adv_set_form", "monc_adv_set_accumulate", "monc_adv_set_pdl", "monc_adv_set_variant",
     "monc_adv_set_tuning", "monc_adv_get_coefficients", "monc_adv_launch_count",
@@ -103,6 +104,8 @@ def load():
     lib.monc_adv_tendencies.restype = ci
     lib.monc_adv_step_async.argtypes = [vp, vp, vp, vp, C.POINTER(vp), ci, vp, vp, vp, C.POINTER(vp), vp]
     lib.monc_adv_step_async.restype = ci
+    lib.monc_adv_step_noalloc.argtypes = [vp] * 8
+    lib.monc_adv_step_noalloc.restype = ci
     for name in ("monc_adv_step_inputs_consumed", "monc_adv_step_wait"):
         getattr(lib, name).argtypes = [vp]
         getattr(lib, name).restype = ci
@@ -260,6 +263,14 @@ class MoncAdv:
         self._step_keepalive = (hu, hv, hw, hq, hsu, hsv, hsw, hsq)
         self._check(self._lib.monc_adv_step_async(self._h, *ins, qp, len(hq), *outs, sp,
                                                   _stream_ptr(stream)))
+
+    def step_noalloc(self, hu, hv, hw, hsu, hsv, hsw, stream=None):
+        """Momentum step from pinned host tensors; device staging in the library's static scratch
+        (no device allocation of any kind; limits and sharing rules: include/monc_adv.h)."""
+        ins = [self._host(t, n) for t, n in zip((hu, hv, hw), ("hu", "hv", "hw"))]
+        outs = [self._host(t, n) for t, n in zip((hsu, hsv, hsw), ("hsu", "hsv", "hsw"))]
+        self._noalloc_keepalive = (hu, hv, hw, hsu, hsv, hsw)
+        self._check(self._lib.monc_adv_step_noalloc(self._h, *ins, *outs, _stream_ptr(stream)))
 
     def step_inputs_consumed(self):
         self._check(self._lib.monc_adv_step_inputs_consumed(self._h))

@@ -1054,6 +1054,65 @@ int step_async_enqueue(monc_adv_t h, const void *hu, const void *hv, const void 
 
 }  // namespace
 
+// ---------------------------------------------------------------------------
+// monc_adv_step_noalloc: the momentum step from pinned host memory with its device staging
+// in a file-scope array instead of cudaMalloc'ed buffers (include/monc_adv.h).
+//
+// g_noalloc_scratch lives in every GPU that loads this library, until exit.  In HOST code
+// its name is a host-side stand-in, not a device address: the address kernels and copies
+// use is fetched with cudaGetSymbolAddress, once per device, with that device current.
+// Every call on a device shares the array (whatever the handle) and finds the last call's
+// contents in it; nothing in it has to start at zero, because a call overwrites every byte
+// its kernel reads (the three whole input arrays) before the kernel runs and copies back
+// only bytes the kernel wrote (interior points of the three tendencies).  Calls that
+// overlap on the GPU (two streams, two host threads) race on it.
+// ---------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MONC_ADV_NOALLOC_MAX_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char *g_noalloc_ptr[kMaxDevices] = {};  // device address of g_noalloc_scratch, per device
+
+// h->device is current (check_handle)
+int noalloc_scratch_address(monc_adv_t h, unsigned char **out) {
+  if (h->device < 0 || h->device >= kMaxDevices) return fail(h, MONC_ADV_EINVAL, "step_noalloc: device ordinal out of range");
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[h->device]) {
+    void *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess || !ptr) {
+      cudaGetLastError();
+      return cuda_fail(h, e == cudaSuccess ? cudaErrorInvalidSymbol : e, "cudaGetSymbolAddress(scratch)");
+    }
+    g_noalloc_ptr[h->device] = static_cast<unsigned char *>(ptr);
+  }
+  *out = g_noalloc_ptr[h->device];
+  return MONC_ADV_OK;
+}
+
+template <typename T>
+int step_noalloc_impl(monc_adv_t h, unsigned char *scratch, size_t slot, const void *hu, const void *hv,
+                      const void *hw, void *hsu, void *hsv, void *hsw, cudaStream_t st) {
+  const size_t bytes = h->elems * sizeof(T);
+  T *d[6];
+  for (int n = 0; n < 6; ++n) d[n] = reinterpret_cast<T *>(scratch + (size_t)n * slot);
+  const void *hin[3] = {hu, hv, hw};
+  void *hout[3] = {hsu, hsv, hsw};
+  for (int n = 0; n < 3; ++n) CU(cudaMemcpyAsync(d[n], hin[n], bytes, cudaMemcpyHostToDevice, st));
+  const int rc = launch_momentum<T>(h, d[0], d[1], d[2], d[3], d[4], d[5], h->h, h->h + h->nx, st);
+  if (rc != MONC_ADV_OK) return rc;
+  // interior columns of the interior planes only: output halos are never written
+  const size_t plane_b = (size_t)h->nyh * h->nz * sizeof(T);
+  const size_t off = ((size_t)h->h * h->nyh + h->h) * h->nz * sizeof(T);
+  const size_t width = (size_t)h->ny * h->nz * sizeof(T);
+  for (int n = 0; n < 3; ++n)
+    CU(cudaMemcpy2DAsync((char *)hout[n] + off, plane_b, (const char *)d[3 + n] + off, plane_b, width, (size_t)h->nx,
+                         cudaMemcpyDeviceToHost, st));
+  return MONC_ADV_OK;
+}
+}  // namespace
+
 extern "C" {
 
 int monc_adv_create(monc_adv_t *out, int nx, int ny, int nz, int halo, double dx, double dy,
@@ -1293,6 +1352,34 @@ int monc_adv_step_async(monc_adv_t h, const void *hu, const void *hv, const void
     h->err = msg;
   }
   return rc;
+}
+
+int monc_adv_step_noalloc(monc_adv_t h, const void *hu, const void *hv, const void *hw, void *hsu, void *hsv,
+                          void *hsw, void *cuda_stream) {
+  int rc = check_handle(h);
+  if (rc) return rc;
+  if (!hu || !hv || !hw || !hsu || !hsv || !hsw) return fail(h, MONC_ADV_EINVAL, "step_noalloc: NULL pointer");
+  if (h->accumulate) return fail(h, MONC_ADV_EINVAL, "step_noalloc: overwrite mode only (set_accumulate(0))");
+  const size_t bytes = h->elems * h->esize;
+  const size_t slot = (bytes + 255) / 256 * 256;  // every staged field starts on a 256-byte boundary
+  if (6 * slot > (size_t)MONC_ADV_NOALLOC_MAX_BYTES) {
+    char b[256];
+    snprintf(b, sizeof b, "step_noalloc: 6 staged fields of %zu bytes need %zu bytes, the static scratch holds "
+             "MONC_ADV_NOALLOC_MAX_BYTES = %zu (use monc_adv_step_async for larger domains)", bytes, 6 * slot,
+             (size_t)MONC_ADV_NOALLOC_MAX_BYTES);
+    return fail(h, MONC_ADV_EINVAL, b);
+  }
+  if (const char *why = find_alias({hu, hv, hw}, {hsu, hsv, hsw}, bytes))
+    return fail(h, MONC_ADV_EINVAL, std::string("step_noalloc: ") + why);
+  for (const void *p : {hu, hv, hw, (const void *)hsu, (const void *)hsv, (const void *)hsw})
+    if (!is_pinned_host(p, bytes))
+      return fail(h, MONC_ADV_EINVAL, "step_noalloc: every host array must be page-locked (pinned) over its whole length");
+  unsigned char *scratch = nullptr;
+  rc = noalloc_scratch_address(h, &scratch);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  return h->dtype == MONC_ADV_F64 ? step_noalloc_impl<double>(h, scratch, slot, hu, hv, hw, hsu, hsv, hsw, st)
+                                  : step_noalloc_impl<float>(h, scratch, slot, hu, hv, hw, hsu, hsv, hsw, st);
 }
 
 int monc_adv_step_inputs_consumed(monc_adv_t h) {
