@@ -450,6 +450,34 @@ def run_device_config(ctx, args, workload, cache, headline):
         rec["sustained"] = {"steps": nsus, "seconds": sms * nsus * 1e-3, "ms_per_step": sms,
                             "value": ctx.world * cfg.points / (sms * 1e-3) / 1e9, "algorithmic_GBs": sg,
                             "frac": sg / roof["peak"], "frac_of_nominal_8TBs": sg / NOMINAL_GBS, "clocks": sclk}
+    # ---- calibration: a plain device copy that moves the same number of bytes per launch (half read, half
+    # written), timed the same way: what this board gives a kernel with no arithmetic, burst and sustained
+    if headline and not swap and ctx.world == 1:
+        try:
+            n8 = int(alg // 16)
+            csrc = [torch.empty(n8, device="cuda", dtype=torch.float64).normal_() for _ in range(2)]
+            cdst = [torch.empty(n8, device="cuda", dtype=torch.float64) for _ in range(2)]
+
+            def copy_step(i):
+                cdst[i % 2].copy_(csrc[i % 2])
+
+            time.sleep(2.0)
+            c0, c1 = timed_loop(ctx, st, copy_step, 20, warm=3)
+            ctx.barrier()
+            cb = c0.elapsed_time(c1) / 20
+            ncs = max(20, int(np.ceil(min(args.sustain_seconds, 1.5) * 1e3 / cb)))
+            c0, c1 = timed_loop(ctx, st, copy_step, ncs)
+            ctx.barrier()
+            cs = c0.elapsed_time(c1) / ncs
+            moved = 2 * n8 * 8
+            rec["copy_same_bytes"] = {"bytes_per_launch": moved, "burst_GBs": moved / (cb * 1e-3) / 1e9,
+                                      "sustained_GBs": moved / (cs * 1e-3) / 1e9, "sustained_steps": ncs,
+                                      "kernel_over_copy_burst": None, "kernel_over_copy_sustained": None,
+                                      "note": "torch copy_ (not this library's kernel), same stream, same event timing"}
+            del csrc, cdst
+            torch.cuda.empty_cache()
+        except Exception as e:  # calibration only
+            rec["copy_same_bytes"] = {"error": f"{type(e).__name__}: {e}"}
     # ---- burst: 20 steps from an idle board, if the headline region was not already that
     if headline and steps > 40 and not swap:
         ctx.barrier()
@@ -929,7 +957,14 @@ def run_ours(args):
            "data": "synthetic", "config": rec["config"], "roofline": rec["roofline"],
            "cpu_baseline": rec.get("cpu_baseline"), "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"],
            "clocks": rec["clocks"]}
-    for k in ("field_points_per_s_G", "sustained", "burst", "two_call_step", "work_scale_16", "accumulate"):
+    c = rec.get("copy_same_bytes")
+    if c and "burst_GBs" in c:
+        if "burst" in rec:
+            c["kernel_over_copy_burst"] = rec["burst"]["algorithmic_GBs"] / c["burst_GBs"]
+        if "sustained" in rec:
+            c["kernel_over_copy_sustained"] = rec["sustained"]["algorithmic_GBs"] / c["sustained_GBs"]
+    for k in ("field_points_per_s_G", "sustained", "burst", "two_call_step", "work_scale_16", "accumulate",
+              "copy_same_bytes"):
         if k in rec:
             out[k] = rec[k]
     if others:
